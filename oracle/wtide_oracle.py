@@ -1,0 +1,363 @@
+"""Plain, slow, double-precision CPU oracle for libwtide.  TEST INFRASTRUCTURE ONLY.
+
+This file restates, step by step and in the paper's order, what the hot path of
+arxiv/paper_2605_13987 computes.  It shares no code with the CUDA path
+(paper_2605_13987_b200/): neither imports the other.  Only tests/,
+__graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import it.  numpy.fft and scipy LU are used as library primitives for single
+steps (a DFT, a dense solve); there is no blocking, fusion or reordering beyond
+what the algorithm states.
+
+What it follows (citations are PAPER.md line + section; "Rn" = reading n listed in
+DESIGN.md, taken from SURVEY.md section 8(c) because the paper defers the PDE to its
+Ref. [10], which is not available):
+
+* Eq. 1.1, PAPER.md:35-39 (section 1):  i(t) = -(q/V_w) int_0^t H(x(t'),t-t').v(t') dt'
+* H solve, PAPER.md:15 (abstract), :65 (section 2), :95, :97 (section 3), Fig. 3 (:109):
+  "fundamental solutions to impose boundary conditions and spectral methods to extend
+  the solution to the bulk", "iterative forward-Euler procedure", V <-> rho through the
+  3-D DFT and |k|^2, V_ext = "rescaled and translated chunks of the fundamental solution".
+
+Pins (tests/test_oracle_*.py, all `-m "not gpu"`): see DESIGN.md section "Oracle pins".
+PARITY UNPINNED: the absolute values of H for the paper's sensor (the paper prints none).
+
+Units (R15): length um, time ns, potential V, charge in elementary charges e.
+H is in V/(um*ns), velocities in um/ns, currents in e/ns.
+"""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+import scipy.linalg
+
+# eps0 = 8.8541878128e-12 F/m  ->  e / (V um)
+EPS0 = 8.8541878128e-12 * 1e-6 / 1.602176634e-19
+WT_BIAS = 0
+WT_READOUT = 1
+
+
+def conductivity(resistivity_ohm_cm: float) -> float:
+    """sigma = 1/resistivity in e/(V um ns).  (1/(ohm cm) = 100 S/m = 1e-4 S/um.)"""
+    return (1.0 / (resistivity_ohm_cm * 1e-2)) * 1e-6 * 1e-9 / 1.602176634e-19
+
+
+def column_resistance_kohm(resistivity_ohm_cm: float, length_um: float, diameter_um: float) -> float:
+    """R = 4 rho L / (pi d^2), PAPER.md:137 (section 5).  Returned in kOhm."""
+    rho_ohm_um = resistivity_ohm_cm * 1e4
+    return 4.0 * rho_ohm_um * length_um / (math.pi * diameter_um ** 2) * 1e-3
+
+
+# ----------------------------------------------------------------------------------------
+# grid, wavenumbers (oracle step 1)
+# ----------------------------------------------------------------------------------------
+def wavenumbers(n: int, length: float):
+    """kappa(k) = 2 pi m / l with m = k for k < n/2, k - n for k > n/2.
+    Returns (kappa[n], retained[n]); the Nyquist index k = n/2 (even n) is not retained (R11)."""
+    k = np.arange(n)
+    m = np.where(2 * k < n, k, k - n).astype(np.float64)
+    retained = np.ones(n, dtype=bool)
+    if n % 2 == 0:
+        retained[n // 2] = False
+        m[n // 2] = 0.0
+    return 2.0 * math.pi * m / length, retained
+
+
+def node_coordinates(n: int, length: float) -> np.ndarray:
+    """x_i = (i * l) / n  (multiply first, then divide: the library uses the same order)."""
+    return (np.arange(n, dtype=np.float64) * length) / n
+
+
+# ----------------------------------------------------------------------------------------
+# voxeliser (oracle step 2; "the STL geometry is voxelized"; R13)
+# ----------------------------------------------------------------------------------------
+def voxelize(desc: dict):
+    """Node-centre test for cylinders parallel to z.
+
+    Returns (col_id[nx,ny,nz] int, sigma[nx,ny,nz], pad_nodes[B,3] int, pad_potential[B], pad_col[B]).
+    A node belongs to column j iff its minimum-image lateral distance^2 to the axis is <= r^2
+    and z0 <= z <= z1; the first column in the list wins on overlap.  Pad nodes of a column =
+    its nodes in its first (pad_at_z1 = 0) or last (pad_at_z1 = 1) z-layer; V_pad = v_w for
+    readout columns, 0 for bias columns (R4, R8).  Pad order: column order, then (ix, iy) row-major.
+    """
+    nx, ny, nz = desc["nx"], desc["ny"], desc["nz"]
+    lx, ly, lz = desc["lx"], desc["ly"], desc["lz"]
+    x = node_coordinates(nx, lx)
+    y = node_coordinates(ny, ly)
+    z = node_coordinates(nz, lz)
+    col_id = np.full((nx, ny, nz), -1, dtype=np.int64)
+    sigma = np.zeros((nx, ny, nz), dtype=np.float64)
+    pad_nodes, pad_pot, pad_col = [], [], []
+    for j, col in enumerate(desc["columns"]):
+        dxm = np.fmod(np.abs(x - col["cx"]), lx)
+        dxm = np.minimum(dxm, lx - dxm)
+        dym = np.fmod(np.abs(y - col["cy"]), ly)
+        dym = np.minimum(dym, ly - dym)
+        inxy = (dxm[:, None] * dxm[:, None] + dym[None, :] * dym[None, :]) <= col["radius"] * col["radius"]
+        inz = (col["z0"] <= z) & (z <= col["z1"])
+        if not inz.any() or not inxy.any():
+            raise ValueError(f"column {j} contains no grid node")
+        member = inxy[:, :, None] & inz[None, None, :] & (col_id < 0)
+        col_id[member] = j
+        sigma[member] = conductivity(col["resistivity"])
+        layers = np.nonzero(inz)[0]
+        kpad = int(layers[-1] if col["pad_at_z1"] else layers[0])
+        ij = np.argwhere(member[:, :, kpad])
+        if len(ij) == 0:
+            raise ValueError(f"column {j} has no pad node")
+        for (i, jj) in ij:
+            pad_nodes.append((int(i), int(jj), kpad))
+            pad_pot.append(desc["v_w"] if col["role"] == WT_READOUT else 0.0)
+            pad_col.append(j)
+    return (col_id, sigma, np.array(pad_nodes, dtype=np.int64).reshape(-1, 3),
+            np.array(pad_pot, dtype=np.float64), np.array(pad_col, dtype=np.int64))
+
+
+def auto_substeps(dt: float, sigma_max: float, eps: float) -> int:
+    """n_sub = ceil(dt * sigma_max / eps)  (R12: dt_int * sigma_max / eps <= 1 < 2 = stability bound)."""
+    return max(1, int(math.ceil(dt * (sigma_max / eps))))
+
+
+# ----------------------------------------------------------------------------------------
+# the quasi-static problem (oracle steps 3-7)
+# ----------------------------------------------------------------------------------------
+class Problem:
+    """div[ eps grad d_t psi + sigma grad psi ] = 0 on a periodic box (R1, R5-R7), pads held
+    at given potentials by point charges on the pad nodes (R8-R10).
+
+    State q[nx,ny,nz] = free charge per node in e (charge density = q / voxel volume).
+    """
+
+    def __init__(self, shape, lengths, eps, sigma, pad_nodes, pad_potential):
+        self.shape = tuple(int(s) for s in shape)
+        self.lengths = tuple(float(l) for l in lengths)
+        self.eps = float(eps)
+        self.sigma = np.asarray(sigma, dtype=np.float64).reshape(self.shape)
+        self.pad_nodes = np.asarray(pad_nodes, dtype=np.int64).reshape(-1, 3)
+        self.pad_potential = np.asarray(pad_potential, dtype=np.float64).reshape(-1)
+        nx, ny, nz = self.shape
+        lx, ly, lz = self.lengths
+        self.vol = (lx / nx) * (ly / ny) * (lz / nz)
+        kx, rx = wavenumbers(nx, lx)
+        ky, ry = wavenumbers(ny, ly)
+        kz, rz = wavenumbers(nz, lz)
+        # step 1: a mode with ANY component at the Nyquist index is removed from every field (R11)
+        self.retained = rx[:, None, None] & ry[None, :, None] & rz[None, None, :]
+        self.kappa = (kx[:, None, None] * self.retained, ky[None, :, None] * self.retained,
+                      kz[None, None, :] * self.retained)
+        k2 = kx[:, None, None] ** 2 + ky[None, :, None] ** 2 + kz[None, None, :] ** 2
+        # step 3: G^(k) = 1/(eps |kappa|^2) on retained non-zero modes, 0 elsewhere
+        self.green_hat = np.zeros(self.shape, dtype=np.float64)
+        ok = self.retained & (k2 > 0)
+        self.green_hat[ok] = 1.0 / (self.eps * k2[ok])
+        # the tabulated fundamental solution (R9): potential of a unit point
+        # charge at node 0 of the periodic lattice, G = IDFT(G^) / voxel volume
+        self.green = np.real(np.fft.ifftn(self.green_hat)) / self.vol
+        # step 4: bordered collocation system  [[G(x_b - x_b'), 1], [1^T, 0]]  (R10)
+        nb = len(self.pad_nodes)
+        self.nb = nb
+        a = np.zeros((nb + 1, nb + 1), dtype=np.float64)
+        for i in range(nb):
+            d = (self.pad_nodes[i][None, :] - self.pad_nodes) % np.array(self.shape)
+            a[i, :nb] = self.green[d[:, 0], d[:, 1], d[:, 2]]
+        a[:nb, nb] = 1.0
+        a[nb, :nb] = 1.0
+        self.bordered = a
+        self._lu = scipy.linalg.lu_factor(a) if nb > 0 else None
+
+    # -- spectral operators (R14, R20) ---------------------------------------------------
+    def grad_s(self, f):
+        """Spectral gradient at the nodes: IDFT(i kappa_a DFT(f)), a = x, y, z."""
+        fh = np.fft.fftn(f)
+        return [np.real(np.fft.ifftn(1j * k * fh)) for k in self.kappa]
+
+    def div_s(self, jx, jy, jz):
+        """Spectral divergence: IDFT(sum_a i kappa_a DFT(J_a))."""
+        acc = np.zeros(self.shape, dtype=np.complex128)
+        for k, j in zip(self.kappa, (jx, jy, jz)):
+            acc += 1j * k * np.fft.fftn(j)
+        return np.real(np.fft.ifftn(acc))
+
+    # -- step 5 ---------------------------------------------------------------------------
+    def potential_of_charge(self, q):
+        """V_rho = IDFT(G^ DFT(q)) / vol: "dividing the spectral representation by |k|^2"."""
+        return np.real(np.fft.ifftn(self.green_hat * np.fft.fftn(q))) / self.vol
+
+    def boundary_charges(self, v_rho, q_total, pad_potential):
+        """Solve A [Q; c] = [V_pad - V_rho|_B ; -sum q]: the point charges "adjusted, in
+        magnitude, to enforce the boundary conditions" (R10)."""
+        if self.nb == 0:
+            return np.zeros(0), 0.0
+        b = self.pad_nodes
+        rhs = np.concatenate([pad_potential - v_rho[b[:, 0], b[:, 1], b[:, 2]], [-q_total]])
+        sol = scipy.linalg.lu_solve(self._lu, rhs)
+        return sol[:-1], float(sol[-1])
+
+    def v_ext(self, charges, c):
+        """V_ext(x) = c + sum_b Q_b G(x - x_b): literal "rescaled and translated chunks of the
+        fundamental solution"."""
+        v = np.full(self.shape, c, dtype=np.float64)
+        for qb, (i, j, k) in zip(charges, self.pad_nodes):
+            v += qb * np.roll(self.green, shift=(int(i), int(j), int(k)), axis=(0, 1, 2))
+        return v
+
+    def potential(self, q, pad_potential=None):
+        """Returns (V, Q, c) with V = V_rho + V_ext."""
+        pp = self.pad_potential if pad_potential is None else np.asarray(pad_potential, dtype=np.float64)
+        v_rho = self.potential_of_charge(q)
+        charges, c = self.boundary_charges(v_rho, float(np.sum(q)), pp)
+        return v_rho + self.v_ext(charges, c), charges, c
+
+    # -- step 7, one forward-Euler substep -------------------------------------------------
+    def euler_substep(self, q, dt_int, pad_potential=None):
+        """V = potential(q); E = -grad_s V; J = sigma E (nodewise, R17); q <- q - dt_int vol div_s J."""
+        v, charges, c = self.potential(q, pad_potential)
+        gx, gy, gz = self.grad_s(v)
+        jx, jy, jz = self.sigma * (-gx), self.sigma * (-gy), self.sigma * (-gz)
+        return q - dt_int * self.vol * self.div_s(jx, jy, jz), charges
+
+    # -- steps 6-8 -------------------------------------------------------------------------
+    def solve_H(self, nt, dt, n_sub, on_substep=None, return_potentials=False, dtype=np.float64):
+        """H[n] = -grad_s(W[n] - W[n-1]) / dt, W[-1] = 0 (R2), W = step response to V_pad Theta(t).
+
+        Returns H[nx,ny,nz,nt,3] (the ABI layout of include/wtide.h) and optionally the list of W[n].
+        """
+        nx, ny, nz = self.shape
+        H = np.zeros((nx, ny, nz, nt, 3), dtype=dtype)
+        q = np.zeros(self.shape, dtype=np.float64)
+        dt_int = dt / n_sub
+        w_prev = np.zeros(self.shape, dtype=np.float64)
+        ws = []
+        for n in range(nt):
+            if n > 0:
+                for s in range(n_sub):
+                    q, charges = self.euler_substep(q, dt_int)
+                    if on_substep is not None:
+                        on_substep(n, s, q, charges)
+            w, _, _ = self.potential(q)
+            g = self.grad_s(w - w_prev)
+            for a in range(3):
+                H[:, :, :, n, a] = -g[a] / dt
+            w_prev = w
+            if return_potentials:
+                ws.append(w)
+        return (H, ws) if return_potentials else H
+
+
+def problem_from_desc(desc: dict) -> Problem:
+    _, sigma, pad_nodes, pad_pot, _ = voxelize(desc)
+    eps = desc["eps_r"] * EPS0
+    return Problem((desc["nx"], desc["ny"], desc["nz"]), (desc["lx"], desc["ly"], desc["lz"]),
+                   eps, sigma, pad_nodes, pad_pot)
+
+
+def substeps_from_desc(desc: dict) -> int:
+    if desc.get("substeps", 0) > 0:
+        return int(desc["substeps"])
+    _, sigma, _, _, _ = voxelize(desc)
+    return auto_substeps(desc["dt"], float(sigma.max()), desc["eps_r"] * EPS0)
+
+
+def solve_H_from_desc(desc: dict, nt=None, dtype=np.float64) -> np.ndarray:
+    prob = problem_from_desc(desc)
+    return prob.solve_H(desc["nt"] if nt is None else nt, desc["dt"], substeps_from_desc(desc), dtype=dtype)
+
+
+# ----------------------------------------------------------------------------------------
+# Eq. 1.1
+# ----------------------------------------------------------------------------------------
+def trajectory_nodes(shape, lengths, pos):
+    """R24 -- the index arithmetic the ABI prescribes, in float32:
+    inv = (float)((double)n / l); u = x * inv (one fp32 multiply); i0 = floor(u); f = u - i0.
+    x, y wrap periodically; z clamps u to [0, nz-1] and i1 = min(i0 + 1, nz - 1).
+    Returns (i0[S,3], i1[S,3], f[S,3] float32, finite[S]).
+    """
+    pos = np.asarray(pos, dtype=np.float32).reshape(-1, 3)
+    i0 = np.zeros(pos.shape, dtype=np.int64)
+    i1 = np.zeros(pos.shape, dtype=np.int64)
+    f = np.zeros(pos.shape, dtype=np.float32)
+    finite = np.isfinite(pos).all(axis=1)
+    safe = np.where(finite[:, None], pos, np.float32(0.0)).astype(np.float32)
+    for a in range(3):
+        n = int(shape[a])
+        inv = np.float32(np.float64(n) / np.float64(lengths[a]))
+        u = (safe[:, a] * inv).astype(np.float32)
+        if a == 2:
+            u = np.minimum(np.maximum(u, np.float32(0.0)), np.float32(n - 1))
+        fl = np.floor(u)
+        f[:, a] = (u - fl).astype(np.float32)
+        ifl = fl.astype(np.int64)
+        if a < 2:
+            i0[:, a] = np.mod(ifl, n)
+            i1[:, a] = np.mod(ifl + 1, n)
+        else:
+            i0[:, a] = ifl
+            i1[:, a] = np.minimum(ifl + 1, n - 1)
+    return i0, i1, f, finite
+
+
+def convolve_currents(H, shape, lengths, nt, dt, v_w, carrier_step_offsets, pos, vel, charge,
+                      track_carrier_offsets=None):
+    """Discrete Eq. 1.1 (R21-R23, R26):
+        i_c[n] = -(q_c / V_w) sum_{m <= n, m < M_c} sum_a H~_a(x_c[m], n - m) v_{c,a}[m] dt
+    H~ = trilinear blend of the 8 surrounding node rows ("linear interpolation along
+    the carrier's trajectory"), indices/fractions by trajectory_nodes (fp32), everything else double.
+    A step whose position or velocity is not finite contributes nothing; steps m >= nt are ignored.
+    Returns i[n_carriers, nt], or i_track[n_tracks, nt] = sum of its carriers in carrier order.
+    """
+    nx, ny, nz = (int(s) for s in shape)
+    Hv = np.asarray(H).reshape(nx, ny, nz, nt, 3)
+    off = np.asarray(carrier_step_offsets, dtype=np.int64)
+    pos = np.asarray(pos, dtype=np.float32).reshape(-1, 3)
+    vel = np.asarray(vel, dtype=np.float32).reshape(-1, 3)
+    charge = np.asarray(charge, dtype=np.float32)
+    n_car = len(off) - 1
+    i0, i1, f, finite = trajectory_nodes(shape, lengths, pos)
+    finite = finite & np.isfinite(vel).all(axis=1)
+    fd = f.astype(np.float64)
+    out = np.zeros((n_car, nt), dtype=np.float64)
+    for c in range(n_car):
+        qc = float(charge[c])
+        for m, s in enumerate(range(off[c], off[c + 1])):
+            if m >= nt:
+                break
+            if not finite[s]:
+                continue
+            row = np.zeros((nt - m, 3), dtype=np.float64)
+            for cx in (0, 1):
+                for cy in (0, 1):
+                    for cz in (0, 1):
+                        w = ((fd[s, 0] if cx else 1.0 - fd[s, 0]) * (fd[s, 1] if cy else 1.0 - fd[s, 1])
+                             * (fd[s, 2] if cz else 1.0 - fd[s, 2]))
+                        ix = i1[s, 0] if cx else i0[s, 0]
+                        iy = i1[s, 1] if cy else i0[s, 1]
+                        iz = i1[s, 2] if cz else i0[s, 2]
+                        row += w * Hv[ix, iy, iz, : nt - m, :].astype(np.float64)
+            v = vel[s].astype(np.float64)
+            out[c, m:] += -(qc / v_w) * (row @ v) * dt
+    if track_carrier_offsets is None:
+        return out
+    toff = np.asarray(track_carrier_offsets, dtype=np.int64)
+    tr = np.zeros((len(toff) - 1, nt), dtype=np.float64)
+    for t in range(len(toff) - 1):
+        for c in range(toff[t], toff[t + 1]):
+            tr[t] += out[c]
+    return tr
+
+
+# error metrics (R27) ---------------------------------------------------------------------
+def h_rel_l2(h_test, h_ref) -> float:
+    a = np.asarray(h_test, dtype=np.float64).ravel()
+    b = np.asarray(h_ref, dtype=np.float64).ravel()
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def current_error(i_test, i_ref):
+    """Per output row: ||di||_2 / (sqrt(nt) max_n |i_ref[n]|); returns (worst row value, max|di|/peak)."""
+    a = np.asarray(i_test, dtype=np.float64)
+    b = np.asarray(i_ref, dtype=np.float64)
+    peak = np.max(np.abs(b), axis=1)
+    peak = np.where(peak > 0, peak, 1.0)
+    l2 = np.linalg.norm(a - b, axis=1) / (math.sqrt(b.shape[1]) * peak)
+    mx = np.max(np.abs(a - b), axis=1) / peak
+    return float(l2.max()), float(mx.max())
