@@ -1,0 +1,149 @@
+/* wtide.h -- C ABI of libwtide (B200 / sm_100a).
+ *
+ * libwtide computes the time-dependent weighting-field correlation function H(x,t) of a 3D
+ * diamond sensor with resistive graphitised column electrodes and evaluates the extended
+ * Ramo-Shockley convolution of arxiv/paper_2605_13987 Eq. 1.1 for batches of drifting carriers.
+ * Citations are PAPER.md line numbers (+ section); "Rn" are the readings listed in DESIGN.md.
+ *
+ * General rules
+ *  - No exceptions, no global state except a thread-local error string (wt_last_error).
+ *  - Return value 0 = WT_OK; negative = error and NO output is written.
+ *  - The library never allocates device memory, never synchronises the stream, never touches the
+ *    default stream.  All device buffers (H tables, trajectories, outputs, workspaces) are
+ *    caller-owned device pointers (e.g. PyTorch tensors' data_ptr()); handles are library-owned
+ *    HOST objects (wt_make_geometry does host work only and needs no GPU).
+ *  - wt_solve_H and wt_convolve_currents ENQUEUE work on `cuda_stream` (a cudaStream_t passed as
+ *    void*; must not be NULL / the legacy default stream) and return at once.  Sticky device
+ *    errors surface at the caller's next synchronisation.
+ *  - Units (R15): length um, time ns, potential V, charge e.  H is V/(um ns), velocity um/ns,
+ *    currents e/ns.
+ *  - H layout is part of the ABI:  H[ ((ix*ny + iy)*nz + iz)*nt + t ][3], fp32, time innermost,
+ *    the three field components interleaved (BASELINE.json north_star (b)).
+ */
+#ifndef WTIDE_H
+#define WTIDE_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define WT_OK         0
+#define WT_EINVAL    -1  /* null pointer, bad size, nt % 4 != 0, grid not 2^a 3^b, offsets not usable      */
+#define WT_EGEOM     -2  /* no readout column, a column without node or pad node, pads of different
+                            potential on one node                                                     */
+#define WT_EUNSTABLE -3  /* `substeps` given and dt/substeps >= 2 eps / sigma_max  (R12)                 */
+#define WT_ENOMEM    -4  /* workspace too small (size via wt_query / wt_conv_workspace_bytes)            */
+#define WT_ECUDA     -5  /* a CUDA call or kernel launch failed                                          */
+
+#define WT_BIAS    0     /* pad held at 0 V                         */
+#define WT_READOUT 1     /* pad stepped to v_w at t = 0  (R2, R4)   */
+
+typedef struct wt_geometry wt_geometry; /* opaque; created by wt_make_geometry, released by wt_free */
+
+/* One graphitised column: a cylinder with its axis parallel to z (Fig. 7). */
+typedef struct {
+  double cx, cy;       /* axis position, um; any value, taken modulo the periodic box            */
+  double radius;       /* um, > 0                                                                */
+  double resistivity;  /* ohm*cm, > 0  (0.75 ohm cm for the test-beam sensor)      */
+  double z0, z1;       /* depth extent, um, 0 <= z0 < z1 <= lz                                   */
+  int    role;         /* WT_BIAS or WT_READOUT                                                  */
+  int    pad_at_z1;    /* 0: the contact pad is the column's first z-layer, 1: its last (R8)     */
+} wt_column;
+
+/* "a text file describing the geometry of the conductive elements" as a C struct. */
+typedef struct {
+  double lx, ly, lz;   /* periodic box, um; lz = sensor thickness (R7)                           */
+  int    nx, ny, nz;   /* grid; node i sits at (i*l)/n; each n = 2^a 3^b, even, 4 <= n <= 1024   */
+  int    nt;           /* time samples of H, a multiple of 4                                      */
+  double dt;           /* ns, output time step of H                                               */
+  double eps_r;        /* relative permittivity (5.7 for diamond), uniform (R5)                   */
+  double v_w;          /* normalisation potential, 1 V                              */
+  int    substeps;     /* forward-Euler substeps per dt; 0 = auto = ceil(dt*sigma_max/eps) (R12)  */
+  int    n_columns;
+  const wt_column* columns; /* host array, borrowed for the duration of the call only            */
+} wt_geometry_desc;
+
+/* Steps a0 (setup) of SURVEY.md section 8(a): voxelise the columns (node-centre test, minimum image
+ * in x,y, first column wins on overlap; R13), collect the pad nodes, build the wavenumber tables,
+ * the mixed-space fundamental-solution tables and the inverse of the bordered collocation matrix
+ * (PAPER.md:64-65 voxelisation; :97 fundamental solution and boundary point charges; R8-R11).
+ * Host work only, fp64.  *out is set only on success. */
+int wt_make_geometry(const wt_geometry_desc* desc, wt_geometry** out);
+
+/* Steps a1-a8: the pseudo-spectral forward-Euler solve of the quasi-static third-order PDE
+ * div[eps grad d_t psi + sigma grad psi] = 0 (Fig. 3; R1-R20) for a
+ * lock-step batch of `n_geoms` geometries on the SAME grid / nt (substeps may differ).
+ *   geoms        host array of n_geoms handles
+ *   H_dev        host array of n_geoms DEVICE pointers; table g receives H in the ABI layout,
+ *                16-byte aligned, H_bytes_each >= WT_Q_H_BYTES
+ *   workspace    device scratch, 256-byte aligned, >= sum over g of WT_Q_SOLVE_WORKSPACE_BYTES
+ * H[n] = -grad_s(W[n] - W[n-1])/dt with W the response to the readout pads stepped to v_w (R2). */
+int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* H_dev, size_t H_bytes_each,
+               void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
+/* Steps a9-a12: Eq. 1.1 discretised on H's time grid (R21-R26):
+ *   i_c[n] = -(q_c/v_w) sum_{m<=n, m<M_c} sum_a H~_a(x_c[m], n-m) v_{c,a}[m] dt,  n < nt,
+ * H~ = trilinear blend of the 8 surrounding node rows with full fp32 weights (R23); indices and
+ * fractions by wt_trajectory_nodes' arithmetic (R24).  Steps m >= nt are ignored (R26); a step
+ * whose position or velocity is not finite contributes nothing.
+ *   track_carrier_offsets_dev [n_tracks+1]   int64, carriers of track t = [off[t], off[t+1])
+ *   carrier_step_offsets_dev  [n_carriers+1] int64, steps of carrier c = [off[c], off[c+1])
+ *   pos_dev, vel_dev          [n_steps][3]   fp32, um and um/ns (v[m] is supplied by the caller, R22)
+ *   charge_dev                [n_carriers]   fp32, e
+ *   per_track 1: out_dev[n_tracks][nt] = sum over the track's carriers in carrier order (fixed
+ *             order, run-to-run deterministic; R25);  0: out_dev[n_carriers][nt]
+ *   workspace >= wt_conv_workspace_bytes(...), 256-byte aligned (may be NULL if that is 0)
+ * Offsets must be non-decreasing with off[0] = 0 (not checked: the arrays live on the device). */
+int wt_convolve_currents(const wt_geometry* geom, const float* H_dev,
+                         int64_t n_tracks, const int64_t* track_carrier_offsets_dev,
+                         int64_t n_carriers, const int64_t* carrier_step_offsets_dev,
+                         const float* pos_dev, const float* vel_dev, const float* charge_dev,
+                         int per_track, float* out_dev,
+                         void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
+/* Releases a handle returned by wt_make_geometry.  NULL is a no-op. */
+void wt_free(void* handle);
+
+/* ---- helpers ------------------------------------------------------------------------------ */
+
+/* Step a9 on its own (R24), for bit-exact index checks:  per step s
+ *   inv = (float)((double)n/l);  u = x*inv (one fp32 multiply);  i0 = floorf(u);  f = u - i0;
+ *   x,y: i0 mod n and (i0+1) mod n;  z: u clamped to [0, nz-1], i1 = min(i0+1, nz-1).
+ * node0_dev[s][3] = (i0x, i0y, i0z), node1_dev[s][3] = (i1x, i1y, i1z), frac_dev[s][3] = f.
+ * A non-finite position gives node0 = node1 = -1 and frac = 0. */
+int wt_trajectory_nodes(const wt_geometry* geom, int64_t n_steps, const float* pos_dev,
+                        int32_t* node0_dev, int32_t* node1_dev, float* frac_dev, void* cuda_stream);
+
+int wt_conv_workspace_bytes(const wt_geometry* geom, int64_t n_tracks, int64_t n_carriers,
+                            int per_track, size_t* bytes);
+
+#define WT_Q_H_BYTES               1  /* nx*ny*nz*nt*3*4                                        */
+#define WT_Q_SOLVE_WORKSPACE_BYTES 2  /* device scratch wt_solve_H needs for THIS geometry       */
+#define WT_Q_SUBSTEPS              3  /* n_sub actually used                                     */
+#define WT_Q_N_PADS                4  /* |B|, number of boundary point charges                   */
+#define WT_Q_N_NODES               5  /* nx*ny*nz                                                */
+#define WT_Q_N_CONDUCTING          6  /* nodes with sigma > 0                                    */
+#define WT_Q_N_PAD_LAYERS          7  /* distinct z-layers holding pads                          */
+#define WT_Q_NT                    8
+int wt_query(const wt_geometry* geom, int what, int64_t* value);
+
+/* Host copies of setup results (for checks against an independent voxeliser):
+ *   WT_A_COLUMN_ID     int8   [nx][ny][nz]   column index of the node, -1 = diamond
+ *   WT_A_PAD_NODES     int32  [B][3]         (ix, iy, iz) in pad order (column, then ix, iy)
+ *   WT_A_PAD_POTENTIAL double [B]
+ * `bytes` must be exactly the array size. */
+#define WT_A_COLUMN_ID     1
+#define WT_A_PAD_NODES     2
+#define WT_A_PAD_POTENTIAL 3
+int wt_get_array(const wt_geometry* geom, int what, void* host_out, size_t bytes);
+
+/* Thread-local description of the last error on this thread ("" if none). */
+const char* wt_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* WTIDE_H */

@@ -1,0 +1,37 @@
+// Internal host-side geometry object of libwtide (not part of the ABI).
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "../../include/wtide.h"
+
+#define WT_MAGIC 0x57544744u /* "WTGD" */
+
+struct wt_geometry {
+  uint32_t magic = WT_MAGIC;
+  // descriptor
+  double lx, ly, lz;
+  int nx, ny, nz, nt;
+  double dt, eps_r, v_w;
+  int n_sub;
+  int n_columns;
+  // setup results (host, fp64)
+  std::vector<int8_t> col_id;       // [nx][ny][nz], -1 = diamond
+  std::vector<double> col_s;        // per column: s = sigma/eps in 1/ns
+  std::vector<int32_t> pad_nodes;   // [B][3]
+  std::vector<double> pad_pot;      // [B]
+  std::vector<int32_t> layers;      // distinct pad z-layers
+  std::vector<int32_t> pad_layer;   // [B] index into layers
+  int64_t n_conducting = 0;
+  // tables uploaded by wt_solve_H (see solve.cu for their use)
+  std::vector<uint8_t> sig_id;      // [z][x][y]: 0 = diamond, j+1 = column j
+  std::vector<float> sdt;           // [256]: s * dt_int of id
+  std::vector<float> gt, gzt;       // [kx][dz][ky] mixed-space fundamental solution and its -d/dz
+  std::vector<double> ainv;         // [B][B] upper-left block of the inverse bordered matrix
+  std::vector<double> kx, ky, kz;   // wavenumbers (0 at the removed Nyquist index); ky has ny/2 entries
+};
+
+void wt_set_error(const std::string& msg);
+bool wt_valid(const wt_geometry* g);
+bool wt_is_2a3b(int n);

@@ -1,0 +1,79 @@
+"""Host-side checks of libwtide that need no GPU: the shared library loads and exports every symbol
+include/wtide.h declares, wt_make_geometry (step a0, host fp64) agrees bit for bit with the oracle's
+voxeliser, and the documented error behaviour holds.  No compute call is made."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2605_13987_b200 as wt
+from oracle import wtide_oracle as wo
+from wtide_inputs import geometry_desc, reduced_desc, sweep_descs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "wtide.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(wt_[a-z_A-Z0-9]+)\s*\(", hdr))
+    assert declared == set(wt.EXPORTS)
+    lib = ctypes.CDLL(wt.LIBRARY_PATH)
+    for name in declared:
+        assert hasattr(lib, name), name
+
+
+@pytest.mark.parametrize("cfg,grid", [(0, None), (1, (32, 32, 16)), (2, (48, 48, 12)), (4, (24, 24, 12))])
+def test_voxeliser_matches_the_oracle_bit_for_bit(cfg, grid):
+    d = geometry_desc(cfg)
+    if grid is not None:
+        d = reduced_desc(d, grid=grid, nt=8)
+    g = wt.wt_make_geometry(d)
+    col_id, sigma, pads, vpad, pcol = wo.voxelize(d)
+    np.testing.assert_array_equal(wt.wt_get_array(g, wt.WT_A_COLUMN_ID), col_id.astype(np.int8))
+    np.testing.assert_array_equal(wt.wt_get_array(g, wt.WT_A_PAD_NODES), pads.astype(np.int32))
+    np.testing.assert_array_equal(wt.wt_get_array(g, wt.WT_A_PAD_POTENTIAL), vpad)
+    assert wt.wt_query(g, wt.WT_Q_SUBSTEPS) == wo.substeps_from_desc(d)
+    assert wt.wt_query(g, wt.WT_Q_N_PADS) == len(pads)
+    assert wt.wt_query(g, wt.WT_Q_N_CONDUCTING) == int((col_id >= 0).sum())
+    assert wt.wt_query(g, wt.WT_Q_H_BYTES) == d["nx"] * d["ny"] * d["nz"] * d["nt"] * 12
+    assert wt.wt_query(g, wt.WT_Q_N_PAD_LAYERS) == len(set(pads[:, 2].tolist()))
+    assert wt.wt_query(g, wt.WT_Q_SOLVE_WORKSPACE_BYTES) > 0
+    wt.wt_free(g)
+    wt.wt_free(g)      # double free through the binding is a no-op
+
+
+def test_sweep_geometries_are_all_valid():
+    """R29: with the swept radius on the bias column all 32 geometries voxelise without overlap errors."""
+    for d in sweep_descs(grid=(32, 32, 8), nt=4):
+        g = wt.wt_make_geometry(d)
+        assert wt.wt_query(g, wt.WT_Q_N_PADS) > 0
+
+
+def test_error_codes():
+    d = reduced_desc(geometry_desc(0), grid=(16, 16, 8), nt=8)
+    bad = dict(d, nt=6)
+    with pytest.raises(wt.WtideError) as e:
+        wt.wt_make_geometry(bad)
+    assert e.value.code == wt.WT_EINVAL
+    with pytest.raises(wt.WtideError) as e:
+        wt.wt_make_geometry(dict(d, nx=20))            # 20 = 2^2 * 5
+    assert e.value.code == wt.WT_EINVAL
+    no_readout = dict(d, columns=[dict(c, role=wt.WT_BIAS) for c in d["columns"]])
+    with pytest.raises(wt.WtideError) as e:
+        wt.wt_make_geometry(no_readout)
+    assert e.value.code == wt.WT_EGEOM
+    thin = dict(d, columns=[dict(d["columns"][0]), dict(d["columns"][1], radius=0.01, cx=1.0, cy=1.0)])
+    with pytest.raises(wt.WtideError) as e:
+        wt.wt_make_geometry(thin)                      # a column that contains no node
+    assert e.value.code == wt.WT_EGEOM
+    with pytest.raises(wt.WtideError) as e:
+        wt.wt_make_geometry(dict(d, substeps=10))      # dt/10 = 1 ps >= 2 tau = 0.5 ps
+    assert e.value.code == wt.WT_EUNSTABLE
+    assert "unstable" in str(e.value)
+    g = wt.wt_make_geometry(dict(d, substeps=25))      # 0.4 ps < 0.5 ps: allowed
+    assert wt.wt_query(g, wt.WT_Q_SUBSTEPS) == 25
+    with pytest.raises(wt.WtideError):
+        wt.wt_query(g, 999)
