@@ -1,0 +1,414 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of libwtide's hot path on BASELINE.json configs[1].
+
+    python bench.py --gpus 1 --steps 3 --warmup 3          # our arm
+    python bench.py --impl reference --steps 1 --warmup 0   # the oracle on the host cores
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: wt_solve_H for the
+config-1 geometry (a0-a8) followed by wt_convolve_currents over all tracks (a9-a12).
+  metric / value : carrier-steps x output-samples per second of the Eq. 1.1 stage (inputs resident in HBM)
+  h_solve_s_per_geometry, stages : the H-solve part of the metric string
+  e2e            : the same Eq. 1.1 throughput with HOST (pinned) trajectory buffers and a host result
+  roofline       : dominant kernel of the step against the measured HBM peak
+  cpu_baseline   : the oracle, as it stands, on a bounded sample of the same workload
+Prints ONE JSON line (rank 0).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "carrier_steps_x_output_samples_per_s"
+UNIT = "terms/s"
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        j = json.load(open(p))
+        return float(j["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def workload(args):
+    from wtide_inputs import geometry_desc, reduced_desc
+    d = geometry_desc(1, seed=0)
+    if args.grid:
+        nx, ny, nz = (int(v) for v in args.grid.split("x"))
+        d = reduced_desc(d, grid=(nx, ny, nz))
+    if args.nt:
+        d = reduced_desc(d, nt=args.nt)
+    return d
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    def __init__(self, index):
+        self.index = index
+        self.samples = []
+        self.reasons = set()
+        self.max_mhz = None
+        self._stop = threading.Event()
+        self._th = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        while not self._stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.index}", f"--query-gpu={q}", "--format=csv,noheader,nounits"],
+                                     capture_output=True, text=True, timeout=5).stdout.strip().split(",")
+                self.samples.append(float(out[0]))
+                self.max_mhz = float(out[1])
+                for n, v in zip(names, out[2:]):
+                    if v.strip().lower().startswith("active"):
+                        self.reasons.add(n)
+            except Exception:  # noqa: BLE001
+                pass
+            self._stop.wait(0.2)
+
+    def __enter__(self):
+        self._th.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        self._th.join(timeout=5)
+
+    def summary(self):
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def count_terms(offsets, nt):
+    """terms = sum_c sum_{m < min(M_c, nt)} (nt - m)"""
+    m = np.minimum(np.diff(np.asarray(offsets, dtype=np.int64)), nt)
+    return int(np.sum(m * nt - m * (m - 1) // 2))
+
+
+# --------------------------------------------------------------------------------------------------
+# oracle legs (CPU): the only places bench.py executes oracle/
+# --------------------------------------------------------------------------------------------------
+def oracle_conv_sample(d, rows_of, csr, budget_s):
+    """Times oracle.convolve_currents carrier chunk by carrier chunk until budget_s is used."""
+    from oracle import wtide_oracle as wo
+    off = np.asarray(csr["carrier_step_offsets"])
+    n_car = len(off) - 1
+    done, terms, t_used, chunk = 0, 0, 0.0, 8
+    while done < n_car and t_used < budget_s:
+        c1 = min(n_car, done + chunk)
+        sub = off[done:c1 + 1] - off[done]
+        sl = slice(off[done], off[c1])
+        t0 = time.perf_counter()
+        wo.convolve_currents(rows_of, (d["nx"], d["ny"], d["nz"]), (d["lx"], d["ly"], d["lz"]), d["nt"], d["dt"], d["v_w"],
+                             sub, csr["pos"][sl], csr["vel"][sl], csr["charge"][done:c1])
+        t_used += time.perf_counter() - t0
+        terms += count_terms(sub, d["nt"])
+        done = c1
+    return terms, t_used, done
+
+
+def oracle_solve_sample(d, budget_s):
+    """Times forward-Euler substeps of the oracle on the workload's grid; returns s per substep."""
+    from oracle import wtide_oracle as wo
+    t0 = time.perf_counter()
+    prob = wo.problem_from_desc(d)
+    n_sub = wo.substeps_from_desc(d)
+    setup = time.perf_counter() - t0
+    q = np.zeros(prob.shape)
+    n, t_used = 0, 0.0
+    while t_used < budget_s or n < 2:
+        t0 = time.perf_counter()
+        q, _ = prob.euler_substep(q, d["dt"] / n_sub)
+        t_used += time.perf_counter() - t0
+        n += 1
+    return t_used / n, n, n_sub, setup
+
+
+def synthetic_host_tracks(d, n_tracks, carriers_per_track, track0=0):
+    """Trajectories for the reference arm without a GPU table: straight saturated drift towards the
+    collecting column (same length statistics as the field drift)."""
+    from wtide_inputs import carriers_on_tracks, make_tracks, straight_drift_cfg0
+    tracks = make_tracks(1, n_tracks + track0, d, 10.0)[track0:]
+    start, sign, charge, toff = carriers_on_tracks(tracks, carriers_per_track, d)
+    return straight_drift_cfg0(d, start, sign, charge, toff, max_steps=d["nt"], speed=100.0)
+
+
+def run_reference(args):
+    """--impl reference: the oracle as it stands on the host cores, bounded sample per step."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    d = workload(args)
+    csr = synthetic_host_tracks(d, 1, 64)
+    rng = np.random.default_rng(0)
+    cache = {}
+
+    def rows_of(ix, iy, iz):      # a synthetic table row (the oracle's arithmetic does not depend on values)
+        key = (ix, iy, iz)
+        if key not in cache:
+            cache[key] = rng.standard_normal((d["nt"], 3)).astype(np.float32)
+        return cache[key]
+    budget = args.ref_budget
+    for _ in range(args.warmup):
+        oracle_conv_sample(d, rows_of, csr, min(1.0, budget))
+    terms = t = 0.0
+    ts = 0.0
+    per_sub = n_sub = None
+    for _ in range(max(1, args.steps)):
+        a, b, ncar = oracle_conv_sample(d, rows_of, csr, budget)
+        terms += a
+        t += b
+        per_sub, nsubs_timed, n_sub, _ = oracle_solve_sample(d, budget)
+        ts += per_sub * nsubs_timed
+    steps = max(1, args.steps)
+    value = terms / t
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * (t + ts) / steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[1] single pixel cell 64x64x256 nt=512 (bounded sample)", "grid": [d["nx"], d["ny"], d["nz"]],
+                       "nt": d["nt"]},
+            "h_solve_s_per_geometry": per_sub * n_sub * (d["nt"] - 1), "h_solve_extrapolated": True,
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle",
+                             "sample": f"{ncar} carriers of one track per step (Eq. 1.1) + {budget:.0f} s of Euler substeps"},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+# --------------------------------------------------------------------------------------------------
+# our arm
+# --------------------------------------------------------------------------------------------------
+def unique_row_bytes(wt, g, csr_dev, nt, n_nodes, chunk_carriers=50_000):
+    """SURVEY 8(d) algorithmic bytes of Eq. 1.1: every distinct (node, lag) element a carrier needs,
+    once: sum over carriers c and visited nodes v of 12 (nt - m_first(c, v)), + 24 M_c + 4 in."""
+    import torch
+    off = csr_dev["carrier_step_offsets"]
+    n_car = off.numel() - 1
+    total = 0
+    for c0 in range(0, n_car, chunk_carriers):
+        c1 = min(n_car, c0 + chunk_carriers)
+        s0, s1 = int(off[c0]), int(off[c1])
+        if s1 == s0:
+            continue
+        pos = csr_dev["pos"][s0:s1]
+        n0, n1, _ = wt.wt_trajectory_nodes(g, pos)
+        lens = (off[c0 + 1:c1 + 1] - off[c0:c1])
+        car = torch.repeat_interleave(torch.arange(c1 - c0, device=pos.device), lens)
+        m = torch.arange(s1 - s0, device=pos.device) - (off[c0:c1] - s0)[car]
+        keep = (m < nt) & (n0[:, 0] >= 0)
+        keys, ms = [], []
+        ny, nz = g.desc["ny"], g.desc["nz"]
+        for cx in (0, 1):
+            for cy in (0, 1):
+                for cz in (0, 1):
+                    ix = (n1 if cx else n0)[:, 0].long()
+                    iy = (n1 if cy else n0)[:, 1].long()
+                    iz = (n1 if cz else n0)[:, 2].long()
+                    keys.append((car * n_nodes + (ix * ny + iy) * nz + iz)[keep])
+                    ms.append(m[keep])
+        keys = torch.cat(keys)
+        ms = torch.cat(ms)
+        uk, inv = torch.unique(keys, return_inverse=True)
+        first = torch.full((uk.numel(),), nt, dtype=torch.int64, device=pos.device)
+        first.scatter_reduce_(0, inv, ms, reduce="amin")
+        total += int((12 * (nt - first)).sum()) + 24 * (s1 - s0) + 4 * (c1 - c0)
+    return total
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+
+    import paper_2605_13987_b200 as wt
+    from wtide_inputs import carriers_on_tracks, field_drift, make_tracks
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    d = workload(args)
+    nt = d["nt"]
+    n_nodes = d["nx"] * d["ny"] * d["nz"]
+    g = wt.wt_make_geometry(d)
+    n_sub = wt.wt_query(g, wt.WT_Q_SUBSTEPS)
+    n_pads = wt.wt_query(g, wt.WT_Q_N_PADS)
+    side = wt._stream(dev)
+
+    # ---- inputs (outside the timed region): the table for the drift field, then the trajectories
+    H = [torch.empty((d["nx"], d["ny"], d["nz"], nt, 3), dtype=torch.float32, device=dev)]
+    ws_solve = torch.empty(wt.wt_query(g, wt.WT_Q_SOLVE_WORKSPACE_BYTES) + 256, dtype=torch.uint8, device=dev)
+    wt.wt_solve_H([g], H=H, workspace=ws_solve, device=dev)
+    torch.cuda.synchronize()
+    e_static = H[0].view(n_nodes, nt, 3).sum(dim=1).mul_(d["dt"]).view(d["nx"], d["ny"], d["nz"], 3)
+    tracks = make_tracks(1, args.tracks * world, d, 10.0)[rank * args.tracks:(rank + 1) * args.tracks]
+    start, sign, charge, toff = carriers_on_tracks(tracks, args.carriers, d)
+    csr = field_drift(e_static, d, start, sign, charge, toff)
+    del e_static
+    torch.cuda.synchronize()
+    off_host = csr["carrier_step_offsets"].cpu().numpy()
+    terms = count_terms(off_host, nt)
+    n_steps_total = int(off_host[-1])
+    n_car = len(off_host) - 1
+    alg_conv_bytes = unique_row_bytes(wt, g, csr, nt, n_nodes) + 4 * nt * args.tracks
+    ws_conv = torch.empty(wt.wt_conv_workspace_bytes(g, args.tracks, n_car, True) + 256, dtype=torch.uint8, device=dev)
+    out = torch.empty((args.tracks, nt), dtype=torch.float32, device=dev)
+
+    def step(ev=None):
+        if ev:
+            ev[0].record(side)
+        wt.wt_solve_H([g], H=H, workspace=ws_solve, device=dev)
+        if ev:
+            ev[1].record(side)
+        wt.wt_convolve_currents(g, H[0], csr["track_carrier_offsets"], csr["carrier_step_offsets"], csr["pos"], csr["vel"],
+                                csr["charge"], per_track=True, out=out, workspace=ws_conv)
+        if ev:
+            ev[2].record(side)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    launches0 = wt.wt_launch_count()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
+    with ClockSampler(local) as clk:
+        t0 = time.perf_counter()
+        for k in range(args.steps):
+            step(evs[k])
+        barrier()
+        wall = time.perf_counter() - t0
+    launches = wt.wt_launch_count() - launches0
+    solve_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
+    conv_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
+    step_ms = float(np.mean([e[0].elapsed_time(e[2]) for e in evs]))
+
+    # ---- e2e: Eq. 1.1 through the C ABI with host buffers (pinned), copies inside the timed region
+    host = {k: v.cpu().pin_memory() for k, v in csr.items()}
+    out_host = torch.empty((args.tracks, nt), dtype=torch.float32).pin_memory()
+    h2d = sum(v.numel() * v.element_size() for v in host.values())
+    d2h = out_host.numel() * 4
+
+    def e2e_step():
+        dv = {k: v.to(dev, non_blocking=True) for k, v in host.items()}
+        wt.wt_convolve_currents(g, H[0], dv["track_carrier_offsets"], dv["carrier_step_offsets"], dv["pos"], dv["vel"],
+                                dv["charge"], per_track=True, out=out, workspace=ws_conv)
+        out_host.copy_(out, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        e2e_step()
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / args.steps
+
+    # ---- reduce over ranks (max time, summed work)
+    vals = torch.tensor([solve_ms, conv_ms, step_ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
+    work = torch.tensor([float(terms)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
+        dist.all_reduce(work, op=dist.ReduceOp.SUM)
+    solve_ms, conv_ms, step_ms, e2e_ms = (float(v) for v in vals.cpu())
+    total_terms = float(work.cpu()[0])
+
+    if rank == 0:
+        peak, peak_kind = measured_peaks()
+        # roofline of the dominant kernel.  Eq. 1.1: algorithmic bytes = per-carrier distinct (node, lag)
+        # elements, duration = CUDA events around wt_convolve_currents on its stream.
+        # H solve: 60 N bytes per Euler substep + 40 N per output step, duration = events
+        # around wt_solve_H.
+        N = n_nodes
+        alg_solve_bytes = (60 * N * n_sub + 40 * N) * (nt - 1) + 40 * N
+        conv_gbs = alg_conv_bytes / (conv_ms * 1e-3) / 1e9
+        solve_gbs = alg_solve_bytes / (solve_ms * 1e-3) / 1e9
+        dominant_is_solve = solve_ms >= conv_ms
+        roof = {"bound": "hbm", "kernel": "wt_solve_H (k_plane + k_spectral + boundary kernels, all substeps)" if dominant_is_solve
+                else "k_conv_carrier", "achieved": solve_gbs if dominant_is_solve else conv_gbs, "peak": peak, "unit": "GB/s",
+                "frac": (solve_gbs if dominant_is_solve else conv_gbs) / peak, "traffic": None, "peak_source": peak_kind,
+                "algorithmic_bytes": alg_solve_bytes if dominant_is_solve else alg_conv_bytes}
+        stages = {"solve_ms": solve_ms, "conv_ms": conv_ms,
+                  "solve": {"algorithmic_bytes": alg_solve_bytes, "achieved_gbs": solve_gbs, "frac": solve_gbs / peak,
+                            "n_sub": n_sub, "substeps": n_sub * (nt - 1), "us_per_substep": 1e3 * solve_ms / (n_sub * (nt - 1)), "pads": n_pads},
+                  "conv": {"algorithmic_bytes": alg_conv_bytes, "no_reuse_gather_bytes": 96 * terms, "achieved_gbs": conv_gbs,
+                           "frac": conv_gbs / peak, "carriers": n_car, "carrier_steps": n_steps_total,
+                           "mean_steps": n_steps_total / max(1, n_car)}}
+        line = {"metric": METRIC, "value": total_terms / (conv_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "configs[1] single pixel cell 55um x 500um, grid %dx%dx%d, nt=%d, dt=%g ns, %d tracks x %d carriers per GPU"
+                           % (d["nx"], d["ny"], d["nz"], nt, d["dt"], args.tracks, args.carriers),
+                           "l2": "inputs larger than L2 (H table %.2f GB, trajectories %.2f GB)" % (n_nodes * nt * 12 / 1e9, n_steps_total * 24 / 1e9),
+                           "parallelism": "replicas, tracks sharded" if world > 1 else "single GPU"},
+                "h_solve_s_per_geometry": solve_ms * 1e-3, "step_value": total_terms / (step_ms * 1e-3), "stages": stages,
+                "roofline": roof,
+                "e2e": {"value": total_terms / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                        "what": "Eq. 1.1 stage with pinned host trajectories in, host currents out"},
+                "gpu_launches": int(launches), "clocks": clk.summary(), "wall_s_timed_region": wall}
+        if not args.no_cpu_baseline and world == 1:
+            # the oracle on a bounded sample of the same workload (first carriers of track 0), rows of
+            # the same fp32 table fetched once
+            ncs = min(n_car, 256)
+            s1 = int(off_host[ncs])
+            sample = {"carrier_step_offsets": off_host[:ncs + 1], "pos": csr["pos"][:s1].cpu().numpy(), "vel": csr["vel"][:s1].cpu().numpy(),
+                      "charge": csr["charge"][:ncs].cpu().numpy()}
+            n0, n1, _ = wt.wt_trajectory_nodes(g, csr["pos"][:s1])
+            ids = set()
+            a0, a1 = n0.cpu().numpy(), n1.cpu().numpy()
+            for cx in (a0, a1):
+                for cy in (a0, a1):
+                    for cz in (a0, a1):
+                        ids.update(zip(cx[:, 0].tolist(), cy[:, 1].tolist(), cz[:, 2].tolist()))
+            ids = [t for t in ids if t[0] >= 0]
+            idx = torch.tensor(ids, device=dev)
+            rows = H[0][idx[:, 0], idx[:, 1], idx[:, 2]].cpu().numpy()
+            table = {t: rows[i] for i, t in enumerate(ids)}
+            o_terms, o_t, o_car = oracle_conv_sample(d, lambda ix, iy, iz: table[(ix, iy, iz)], sample, args.ref_budget)
+            per_sub, nsubs, _, _ = oracle_solve_sample(d, args.ref_budget)
+            line["cpu_baseline"] = {"value": o_terms / o_t, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "sample": "%d carriers of track 0 (%.1f s) for Eq. 1.1; %d Euler substeps on the full grid (%.2f s each) "
+                                              "-> H solve extrapolated to %.0f s per geometry" % (o_car, o_t, nsubs, per_sub, per_sub * n_sub * (nt - 1)),
+                                    "h_solve_s_per_geometry_extrapolated": per_sub * n_sub * (nt - 1), "host_cores_available": os.cpu_count()}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--tracks", type=int, default=1000, help="MIP tracks per GPU")
+    ap.add_argument("--carriers", type=int, default=1000, help="macro-carriers per track")
+    ap.add_argument("--grid", default="", help="override grid, e.g. 32x32x64 (debug only; not a bench line)")
+    ap.add_argument("--nt", type=int, default=0, help="override nt (debug only)")
+    ap.add_argument("--ref-budget", type=float, default=10.0, help="seconds of oracle work per leg")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -140,6 +140,10 @@ int wt_query(const wt_geometry* geom, int what, int64_t* value);
 #define WT_A_PAD_POTENTIAL 3
 int wt_get_array(const wt_geometry* geom, int what, void* host_out, size_t bytes);
 
+/* Number of CUDA kernels this process has launched through libwtide so far (bench.py reports the
+ * difference over its timed region as "gpu_launches"). */
+int64_t wt_launch_count(void);
+
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* wt_last_error(void);
 

@@ -304,9 +304,17 @@ def convolve_currents(H, shape, lengths, nt, dt, v_w, carrier_step_offsets, pos,
     the carrier's trajectory"), indices/fractions by trajectory_nodes (fp32), everything else double.
     A step whose position or velocity is not finite contributes nothing; steps m >= nt are ignored.
     Returns i[n_carriers, nt], or i_track[n_tracks, nt] = sum of its carriers in carrier order.
+    H is the table [nx,ny,nz,nt,3] or a callable H(ix, iy, iz) -> row [nt,3] (for tables that do not
+    fit in host memory; only data access, no arithmetic).
     """
     nx, ny, nz = (int(s) for s in shape)
-    Hv = np.asarray(H).reshape(nx, ny, nz, nt, 3)
+    if callable(H):
+        rows_of = H
+    else:
+        Hv = np.asarray(H).reshape(nx, ny, nz, nt, 3)
+
+        def rows_of(ix, iy, iz):
+            return Hv[ix, iy, iz]
     off = np.asarray(carrier_step_offsets, dtype=np.int64)
     pos = np.asarray(pos, dtype=np.float32).reshape(-1, 3)
     vel = np.asarray(vel, dtype=np.float32).reshape(-1, 3)
@@ -332,7 +340,7 @@ def convolve_currents(H, shape, lengths, nt, dt, v_w, carrier_step_offsets, pos,
                         ix = i1[s, 0] if cx else i0[s, 0]
                         iy = i1[s, 1] if cy else i0[s, 1]
                         iz = i1[s, 2] if cz else i0[s, 2]
-                        row += w * Hv[ix, iy, iz, : nt - m, :].astype(np.float64)
+                        row += w * np.asarray(rows_of(int(ix), int(iy), int(iz)))[: nt - m, :].astype(np.float64)
             v = vel[s].astype(np.float64)
             out[c, m:] += -(qc / v_w) * (row @ v) * dt
     if track_carrier_offsets is None:

@@ -21,7 +21,7 @@ WT_Q_N_NODES, WT_Q_N_CONDUCTING, WT_Q_N_PAD_LAYERS, WT_Q_NT = 5, 6, 7, 8
 WT_A_COLUMN_ID, WT_A_PAD_NODES, WT_A_PAD_POTENTIAL = 1, 2, 3
 
 EXPORTS = ("wt_make_geometry", "wt_solve_H", "wt_convolve_currents", "wt_free", "wt_trajectory_nodes",
-           "wt_conv_workspace_bytes", "wt_query", "wt_get_array", "wt_last_error")
+           "wt_conv_workspace_bytes", "wt_query", "wt_get_array", "wt_last_error", "wt_launch_count")
 
 
 class wt_column(C.Structure):
@@ -62,6 +62,7 @@ def _load():
     lib.wt_query.argtypes = [vp, C.c_int, C.POINTER(i64)]
     lib.wt_get_array.argtypes = [vp, C.c_int, vp, sz]
     lib.wt_last_error.restype = C.c_char_p
+    lib.wt_launch_count.restype = C.c_int64
     for n in ("wt_make_geometry", "wt_solve_H", "wt_convolve_currents", "wt_trajectory_nodes",
               "wt_conv_workspace_bytes", "wt_query", "wt_get_array"):
         getattr(lib, n).restype = C.c_int
@@ -218,6 +219,10 @@ def wt_convolve_currents(geom, H, track_carrier_offsets, carrier_step_offsets, p
         if t is not None:
             t.record_stream(_stream(device))
     return out
+
+
+def wt_launch_count() -> int:
+    return int(_lib.wt_launch_count())
 
 
 def wt_trajectory_nodes(geom, pos):

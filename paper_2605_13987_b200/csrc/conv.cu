@@ -86,8 +86,10 @@ __global__ void __launch_bounds__(kThreads) k_conv_carrier(ConvParams p) {
           const float w = (cx ? nf.f[0] : 1.f - nf.f[0]) * (cy ? nf.f[1] : 1.f - nf.f[1]) * (cz ? nf.f[2] : 1.f - nf.f[2]);
           const int ix = cx ? nf.i1[0] : nf.i0[0], iy = cy ? nf.i1[1] : nf.i0[1], iz = cz ? nf.i1[2] : nf.i0[2];
           node[threadIdx.x][k] = ok ? (unsigned)((ix * p.ny + iy) * p.nz + iz) : 0u;
-          const float ws = ok ? w * scale : 0.f;
-          coef[threadIdx.x][k][0] = ws * vx; coef[threadIdx.x][k][1] = ws * vy; coef[threadIdx.x][k][2] = ws * vz;
+          const float ws = w * scale;     // a non-finite step contributes nothing (0, not 0 * inf)
+          coef[threadIdx.x][k][0] = ok ? ws * vx : 0.f;
+          coef[threadIdx.x][k][1] = ok ? ws * vy : 0.f;
+          coef[threadIdx.x][k][2] = ok ? ws * vz : 0.f;
         }
       }
       __syncthreads();
@@ -174,7 +176,9 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
   p.nx = g->nx; p.ny = g->ny; p.nz = g->nz; p.nt = g->nt;
   p.invx = (float)((double)g->nx / g->lx); p.invy = (float)((double)g->ny / g->ly); p.invz = (float)((double)g->nz / g->lz);
   p.dt_over_vw = (float)(g->dt / g->v_w);
+  if (n_carriers > 0) ++g_wt_launches;
   if (n_carriers > 0) k_conv_carrier<<<(unsigned)n_carriers, kThreads, 0, st>>>(p);
+  if (per_track && n_tracks > 0) ++g_wt_launches;
   if (per_track && n_tracks > 0)
     k_track_sum<<<(unsigned)n_tracks, 256, 0, st>>>((const float*)workspace_dev, track_carrier_offsets_dev, out_dev, g->nt);
   cudaError_t e = cudaGetLastError();
@@ -188,6 +192,7 @@ extern "C" int wt_trajectory_nodes(const wt_geometry* g, int64_t n_steps, const 
   if (!wt_valid(g) || n_steps < 0 || !cuda_stream || (n_steps > 0 && (!pos_dev || !node0_dev || !node1_dev || !frac_dev))) {
     wt_set_error("wt_trajectory_nodes: bad argument"); return WT_EINVAL;
   }
+  if (n_steps > 0) ++g_wt_launches;
   if (n_steps > 0)
     k_nodes<<<(unsigned)((n_steps + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(
         n_steps, pos_dev, node0_dev, node1_dev, frac_dev, g->nx, g->ny, g->nz, (float)((double)g->nx / g->lx),

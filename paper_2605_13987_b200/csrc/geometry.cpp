@@ -11,6 +11,8 @@
 #include <cstring>
 
 static thread_local std::string g_err;
+std::atomic<long long> g_wt_launches{0};
+extern "C" int64_t wt_launch_count(void) { return (int64_t)g_wt_launches.load(); }
 void wt_set_error(const std::string& msg) { g_err = msg; }
 extern "C" const char* wt_last_error(void) { return g_err.c_str(); }
 bool wt_valid(const wt_geometry* g) { return g != nullptr && g->magic == WT_MAGIC; }

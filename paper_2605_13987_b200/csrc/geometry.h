@@ -1,5 +1,6 @@
 // Internal host-side geometry object of libwtide (not part of the ABI).
 #pragma once
+#include <atomic>
 #include <cstdint>
 #include <string>
 #include <vector>
@@ -32,6 +33,7 @@ struct wt_geometry {
   std::vector<double> kx, ky, kz;   // wavenumbers (0 at the removed Nyquist index); ky has ny/2 entries
 };
 
+extern std::atomic<long long> g_wt_launches;   // kernels launched by this process (wt_launch_count)
 void wt_set_error(const std::string& msg);
 bool wt_valid(const wt_geometry* g);
 bool wt_is_2a3b(int n);

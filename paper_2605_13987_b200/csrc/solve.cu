@@ -596,6 +596,7 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
 
   auto boundary = [&](int s, int emit, double flag) {
     if (maxB == 0) return;
+    g_wt_launches += 3;
     k_rhs<<<g_warpB, 256, 0, st>>>(gd, dgeoms, s, emit, flag);
     k_matvec<<<g_warpB, 256, 0, st>>>(dgeoms, s);
     k_inject<<<g_inj, 256, 0, st>>>(gd, dgeoms, s);
@@ -603,16 +604,19 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   auto emit_step = [&](int n) {
     // H[n] from the increment of the charge since the previous output step (the prompt response
     // H[0] from the pads alone: r = 0, pads at v_w)
+    g_wt_launches += 2;
     if (n == 0) k_spectral<false, false><<<g_spec, b_spec, sm_spec, st>>>(gd, dgeoms, 0, 1);
     else        k_spectral<false, true><<<g_spec, b_spec, sm_spec, st>>>(gd, dgeoms, 0, 1);
     boundary(0, 1, n == 0 ? 1.0 : 0.0);
     k_plane<true><<<g_plane, 256, sm_plane, st>>>(gd, dgeoms, 0, n % kStageSlots);
     if ((n + 1) % kStageSlots == 0 || n == nt - 1) {
       const int cnt = n % kStageSlots + 1, t0 = n - cnt + 1;
+      ++g_wt_launches;
       k_transpose<<<g_tr, 256, (size_t)cnt * 3 * ny * sizeof(float), st>>>(gd, dgeoms, t0, cnt);
     }
   };
 
+  g_wt_launches += 2 * n_geoms + 1;
   for (int i = 0; i < n_geoms; ++i) {
     k_zero<<<(unsigned)((half + 255) / 256), 256, 0, st>>>(hd[i].rhat, half);
     k_zero<<<(unsigned)((half + 255) / 256), 256, 0, st>>>(hd[i].rhat_prev, half);
@@ -623,6 +627,7 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   for (int n = 1; n < nt; ++n) {
     for (int s = 0; s < max_sub; ++s) {
       boundary(s, 0, 1.0);
+      g_wt_launches += 2;
       k_plane<false><<<g_plane, 256, sm_plane, st>>>(gd, dgeoms, s, 0);
       k_spectral<true, false><<<g_spec, b_spec, sm_spec, st>>>(gd, dgeoms, s, 0);
     }

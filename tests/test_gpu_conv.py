@@ -1,0 +1,147 @@
+"""GPU parity of wt_convolve_currents / wt_trajectory_nodes (steps a9-a12) against the oracle,
+element by element on the same seeded inputs, through the C ABI.
+
+Tolerance (north_star / R27): currents within 2e-4 of the oracle, normalised to the row's peak;
+indices bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+import paper_2605_13987_b200 as wt
+from oracle import wtide_oracle as wo
+from wtide_inputs import (carriers_on_tracks, geometry_desc, make_tracks, reduced_desc,
+                          straight_drift_cfg0)
+
+pytestmark = pytest.mark.gpu
+TOL = 2e-4
+DEV = "cuda:0"
+
+
+def _to_dev(csr):
+    return {k: torch.as_tensor(np.asarray(v)).to(DEV) for k, v in csr.items()}
+
+
+def _run(g, H, csr, per_track):
+    c = _to_dev(csr)
+    out = wt.wt_convolve_currents(g, H, c["track_carrier_offsets"], c["carrier_step_offsets"], c["pos"], c["vel"],
+                                  c["charge"], per_track=per_track)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def _oracle(d, Hnp, csr, per_track):
+    return wo.convolve_currents(Hnp, (d["nx"], d["ny"], d["nz"]), (d["lx"], d["ly"], d["lz"]), d["nt"], d["dt"], d["v_w"],
+                                csr["carrier_step_offsets"], csr["pos"], csr["vel"], csr["charge"],
+                                csr["track_carrier_offsets"] if per_track else None)
+
+
+def test_trajectory_nodes_bit_exact():
+    d = geometry_desc(1)
+    g = wt.wt_make_geometry(reduced_desc(d, grid=(64, 64, 256), nt=8, substeps=100))
+    rng = np.random.default_rng(0)
+    pos = rng.uniform(-200.0, 700.0, size=(200_000, 3)).astype(np.float32)
+    pos[:1000] = rng.uniform(0, 55.0, size=(1000, 3)).astype(np.float32)
+    pos[5] = [np.nan, 1, 1]
+    pos[6] = [1, np.inf, 1]
+    # exact node positions and cell boundaries
+    pos[1000:1064, 0] = (np.arange(64) * 55.0 / 64).astype(np.float32)
+    n0, n1, fr = wt.wt_trajectory_nodes(g, torch.as_tensor(pos).to(DEV))
+    torch.cuda.synchronize()
+    i0, i1, f, fin = wo.trajectory_nodes((64, 64, 256), (55.0, 55.0, 500.0), pos)
+    n0, n1, fr = n0.cpu().numpy(), n1.cpu().numpy(), fr.cpu().numpy()
+    assert np.array_equal(n0[fin], i0[fin].astype(np.int32))
+    assert np.array_equal(n1[fin], i1[fin].astype(np.int32))
+    assert np.array_equal(fr[fin].view(np.uint32), f[fin].view(np.uint32))       # bit-exact fractions
+    assert (n0[~fin] == -1).all() and (n1[~fin] == -1).all()
+
+
+def test_cfg0_currents_match_the_oracle():
+    """Config 0 workload (256 carriers on one perpendicular track, straight drift, R28) on a random
+    fp32 table (conv parity is decoupled from solver parity): per-carrier and per-track outputs."""
+    d = geometry_desc(0)
+    g = wt.wt_make_geometry(d)
+    rng = np.random.default_rng(1)
+    Hnp = rng.standard_normal((d["nx"], d["ny"], d["nz"], d["nt"], 3)).astype(np.float32)
+    H = torch.as_tensor(Hnp).to(DEV)
+    tracks = make_tracks(0, 1, d, 0.0)
+    start, sign, charge, toff = carriers_on_tracks(tracks, 256, d, unit_charge=True)
+    csr = straight_drift_cfg0(d, start, sign, charge, toff)
+    assert csr["carrier_step_offsets"][-1] > 1000
+    for per_track in (False, True):
+        got = _run(g, H, csr, per_track)
+        ref = _oracle(d, Hnp, csr, per_track)
+        l2, mx = wo.current_error(got, ref)
+        assert l2 <= TOL and mx <= 5 * TOL, (per_track, l2, mx)
+
+
+def test_ragged_and_degenerate_inputs():
+    """Empty carriers, a carrier longer than nt (R26), steps outside the box, non-finite steps,
+    a track without carriers, several tiles of outputs (nt = 1024 > 512 per tile) and nt = 4."""
+    for nt in (1024, 4, 36):
+        d = reduced_desc(geometry_desc(0), grid=(12, 8, 6), nt=nt)
+        g = wt.wt_make_geometry(d)
+        rng = np.random.default_rng(nt)
+        Hnp = rng.standard_normal((12, 8, 6, nt, 3)).astype(np.float32)
+        H = torch.as_tensor(Hnp).to(DEV)
+        lens = [0, 3, nt + 7, 1, 0, 40, 5, 0]
+        off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+        S = int(off[-1])
+        pos = rng.uniform(-100, 150, size=(S, 3)).astype(np.float32)
+        vel = rng.standard_normal((S, 3)).astype(np.float32)
+        pos[off[2] + 1, 1] = np.nan
+        vel[off[5] + 2, 0] = np.inf
+        csr = dict(track_carrier_offsets=np.array([0, 1, 1, 4, 8], np.int64), carrier_step_offsets=off, pos=pos, vel=vel,
+                   charge=rng.standard_normal(len(lens)).astype(np.float32))
+        for per_track in (False, True):
+            got = _run(g, H, csr, per_track)
+            ref = _oracle(d, Hnp, csr, per_track)
+            assert np.isfinite(got).all()
+            scale = np.abs(ref).max()
+            assert np.abs(got - ref).max() <= TOL * scale, (nt, per_track)
+            if per_track:
+                assert (got[1] == 0).all()
+    # zero carriers / zero tracks: a valid call that writes nothing
+    out = wt.wt_convolve_currents(g, H, torch.zeros(1, dtype=torch.int64, device=DEV), torch.zeros(1, dtype=torch.int64, device=DEV),
+                                  torch.zeros((0, 3), device=DEV), torch.zeros((0, 3), device=DEV), torch.zeros(0, device=DEV))
+    assert out.shape == (0, nt)
+
+
+def test_run_to_run_determinism():
+    d = reduced_desc(geometry_desc(0), grid=(16, 16, 8), nt=64)
+    g = wt.wt_make_geometry(d)
+    H = torch.randn((16, 16, 8, 64, 3), device=DEV)
+    tracks = make_tracks(0, 4, d, 5.0)
+    start, sign, charge, toff = carriers_on_tracks(tracks, 64, d)
+    csr = straight_drift_cfg0(d, start, sign, charge, toff, max_steps=64)
+    a = _run(g, H, csr, True)
+    b = _run(g, H, csr, True)
+    assert np.array_equal(a.view(np.uint32), b.view(np.uint32))
+
+
+def test_full_size_table_sampled_tracks():
+    """BASELINE.json configs[1] sizes (64x64x256 grid, nt = 512, 6.4 GB table) in the launch
+    configuration bench.py times; the oracle computes a sample of tracks from rows fetched on demand."""
+    d = geometry_desc(1)
+    g = wt.wt_make_geometry(reduced_desc(d, substeps=100))
+    gen = torch.Generator(device=DEV).manual_seed(3)
+    H = torch.randn((64, 64, 256, 512, 3), device=DEV, generator=gen)
+    tracks = make_tracks(1, 3, d, 10.0)
+    start, sign, charge, toff = carriers_on_tracks(tracks, 40, d)
+    # curved synthetic paths of ragged length (the solver-driven drift is exercised in test_gpu_solve)
+    rng = np.random.default_rng(5)
+    lens = rng.integers(0, 90, size=len(start))
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    pos = np.concatenate([start[c] + np.cumsum(rng.normal(0.3, 0.3, size=(lens[c], 3)), axis=0) for c in range(len(start))]).astype(np.float32)
+    vel = rng.standard_normal((int(off[-1]), 3)).astype(np.float32) * 100
+    csr = dict(track_carrier_offsets=toff, carrier_step_offsets=off, pos=pos, vel=vel, charge=charge)
+    got = _run(g, H, csr, True)
+    cache = {}
+
+    def rows(ix, iy, iz):
+        key = (ix, iy, iz)
+        if key not in cache:
+            cache[key] = H[ix, iy, iz].cpu().numpy()
+        return cache[key]
+    ref = _oracle(d, rows, csr, True)
+    l2, mx = wo.current_error(got, ref)
+    assert l2 <= TOL and mx <= 5 * TOL, (l2, mx)
