@@ -158,8 +158,9 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
                                     const float* charge_dev, int per_track, float* out_dev, void* workspace_dev,
                                     size_t workspace_bytes, void* cuda_stream) {
   if (!wt_valid(g)) { wt_set_error("wt_convolve_currents: bad handle"); return WT_EINVAL; }
-  if (!H_dev || !carrier_step_offsets_dev || !charge_dev || !out_dev || !cuda_stream || n_carriers < 0 || n_tracks < 0 ||
-      (per_track && !track_carrier_offsets_dev)) {
+  const int64_t rows = per_track ? n_tracks : n_carriers;
+  if (!H_dev || !carrier_step_offsets_dev || (!charge_dev && n_carriers > 0) || (!out_dev && rows > 0) || !cuda_stream ||
+      n_carriers < 0 || n_tracks < 0 || (per_track && !track_carrier_offsets_dev)) {
     wt_set_error("wt_convolve_currents: null argument, negative count or NULL (default) stream"); return WT_EINVAL;
   }
   if (n_carriers > 0x7fffffffLL || n_tracks > 0x7fffffffLL) { wt_set_error("wt_convolve_currents: more than 2^31-1 carriers or tracks in one call"); return WT_EINVAL; }
