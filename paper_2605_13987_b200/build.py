@@ -8,7 +8,8 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SOURCES = ["csrc/geometry.cpp", "csrc/solve.cu", "csrc/conv.cu"]
-DEPS = SOURCES + ["csrc/fft.cuh", "csrc/geometry.h", "../include/wtide.h"]
+DEPS = SOURCES + ["csrc/fft.cuh", "csrc/regfft.cuh", "csrc/solve_common.cuh", "csrc/solve_boundary.cuh",
+                  "csrc/solve_generic.cuh", "csrc/solve_fast.cuh", "csrc/geometry.h", "../include/wtide.h"]
 LIB = os.path.join(HERE, "libwtide.so")
 
 

@@ -3,415 +3,41 @@
 // Method (Fig. 3 :109; readings R1-R20 of DESIGN.md): forward Euler on
 //   r <- r - dt_int div_s( s E ),  E = -grad_s V,  V = (r + boundary charges)/|kappa|^2 ,
 // in units eps = 1 (r = rho/eps, s = sigma/eps).  The 3-D DFT is split into z-line transforms
-// (k_spectral, one CTA per (kx, tile of ky)) and xy-plane transforms (k_plane, one CTA per z);
-// the fields between them live in "mixed space" arrays M[kx][z][ky] (ky >= 0 half spectrum).
+// (one CTA per (kx, tile of ky)) and xy-plane transforms (one CTA per z); the fields between them
+// live in "mixed space" arrays M[kx][z][ky] (ky >= 0 half spectrum).
 //
 // One Euler substep =
-//   k_rhs      pad potentials from the free charge (partials written by k_spectral) -> rhs      (a3)
-//   k_matvec   Q' = Ainv rhs: "adjusted, in magnitude, to enforce the boundary conditions"       (a3)
-//   k_inject   spectrum of the boundary point charges per pad layer                              (a4)
-//   k_plane    V~ = V~_rho + sum_l Q^_l * g~ (translated fundamental solution, a4); E~ = -i kappa V~;
+//   k_padpot   pad potentials of the free charge from pl = V~_rho at the pad layers -> rhs           (a3)
+//   k_matvec   Q' = Ainv rhs: "adjusted, in magnitude, to enforce the boundary conditions"          (a3)
+//   k_inject   spectrum of the boundary point charges per pad layer                                 (a4)
+//   plane      V~ = V~_rho + sum_l Q^_l * g~ (translated fundamental solution, a4); E~ = -i kappa V~;
 //              inverse xy DFT (a5); J = s dt_int E (a6); forward xy DFT; D~ = i kx J~x + i ky J~y
-//   k_spectral forward z DFT; r^ -= D^ + i kz J^z (a7, fp64 state); V^ = r^/|kappa|^2 (a2);
-//              pad-layer potentials (fp64); inverse z DFT of V^ and -i kz V^
+//   z-line     forward z DFT; r^ -= D^ + i kz J^z (a7, fp64 state); V^ = r^/|kappa|^2 (a2);
+//              pl (fp64); inverse z DFT of V^ and -i kz V^
 // Every n_sub substeps the same kernels run once on the increment r^ - r^_prev with the pads at
 // 0 V and write H[n] = E/dt (a8) through a staging buffer that turns the time-innermost table
-// writes into 12*TB-byte runs (k_transpose).
+// writes into 12*TB-byte runs (k_transpose).  The kernels of one output step (n_sub substeps + emit)
+// are captured once into a CUDA graph and replayed nt-1 times; the output-step index lives in a
+// device counter.  Plane and z-line kernels come in a size-generic family (solve_generic.cuh) and a
+// register-FFT family for power-of-two sizes (solve_fast.cuh).
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
+#include <map>
 #include <string>
 #include <vector>
 
-#include "fft.cuh"
 #include "geometry.h"
+#include "solve_boundary.cuh"
+#include "solve_fast.cuh"
+#include "solve_generic.cuh"
 
 namespace {
+using namespace wt;
 
-constexpr int kMaxLayers = 8;
-constexpr int kStageSlots = 8;   // TB: output steps buffered before a table write (96-byte runs)
-
-struct GridDev {
-  int nx, ny, nz, y2, nt, ty, n_tiles;   // n_tiles = nx * (y2/ty) = CTAs of k_spectral per geometry
-  double inv_n;
-};
-
-struct GeomDev {
-  // static tables
-  const uint8_t* sig_id;     // [z][x][y]
-  const float* sdt;          // [256]
-  const float* gt;           // [kx][dz][ky]
-  const float* gzt;
-  const double* ainv;        // [B][B]
-  const int* pad_x; const int* pad_y; const int* pad_layer;   // [B]
-  const double* pad_pot;     // [B]
-  const int* layer_off;      // [L+1] offsets into layer_idx
-  const int* layer_idx;      // [B] pad indices grouped by layer
-  const double* kxd; const double* kyd; const double* kzd;    // wavenumbers
-  const float2* twx; const float2* twy; const float2* twz;    // e^{-2 pi i k/n}
-  const double2* twxd; const double2* twyd; const double2* twzd;
-  // state
-  double2* rhat; double2* rhat_prev;   // [kx][kz][ky]
-  float2* m0; float2* m1;              // step pipeline: (V~_rho | D~), (E~z_rho | J~z)   [kx][z][ky]
-  float2* e0; float2* e1;              // emit pipeline
-  double* part; double* part_e;        // [n_tiles][B] pad-potential partials
-  double* rhs; double* q;              // [B]
-  float2* qh;                          // [L][kx][ky] spectrum of the boundary charges
-  float* stage;                        // [TB][3][z][x][y]
-  float* H;
-  int layers[kMaxLayers];
-  int B, L, n_sub;
-  float inv_dt;
-};
-
-__device__ __forceinline__ double2 dmul(double2 a, double2 b) {
-  return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
-}
-
-// ------------------------------------------------------------------------------------------------
-// k_spectral: z-line transforms + per-mode update.  grid (n_tiles, n_geoms), block 32*ty.
-// ------------------------------------------------------------------------------------------------
-template <bool APPLY_J, bool DELTA>
-__global__ void __launch_bounds__(256) k_spectral(GridDev gd, const GeomDev* __restrict__ geoms, int substep, int emit) {
-  const GeomDev& g = geoms[blockIdx.y];
-  if (substep >= g.n_sub) return;
-  const int nx = gd.nx, nz = gd.nz, y2 = gd.y2, TY = gd.ty;
-  const int tiles = y2 / TY;
-  const int kx = blockIdx.x / tiles, ky0 = (blockIdx.x % tiles) * TY;
-  const int tid = threadIdx.x, bd = blockDim.x;
-  const int nelem = nz * TY;
-  const int L = g.L, B = g.B;
-  extern __shared__ __align__(16) unsigned char smraw[];
-  float2* b0 = reinterpret_cast<float2*>(smraw);
-  float2* b1 = b0 + nelem;
-  float2* b2 = b1 + nelem;
-  double2* red = reinterpret_cast<double2*>(b2 + nelem);   // [L][TY][32]
-  double2* pl = red + L * TY * 32;                          // [L][TY]
-  float2* mV = emit ? g.e0 : g.m0;
-  float2* mE = emit ? g.e1 : g.m1;
-  const size_t slab = (size_t)kx * nz * y2 + ky0;
-
-  float2 *dres, *jres, *vb;
-  if (APPLY_J) {
-    for (int t = tid; t < nelem; t += bd) {
-      const int z = t / TY, ty = t - z * TY;
-      const size_t gi = slab + (size_t)z * y2 + ty;
-      b0[t] = g.m0[gi];
-      b2[t] = g.m1[gi];
-    }
-    __syncthreads();
-    dres = wt::fft_lines<float2>(b0, b1, nz, TY, 1, TY, g.twz, false);
-    float2* free1 = (dres == b0) ? b1 : b0;
-    jres = wt::fft_lines<float2>(b2, free1, nz, TY, 1, TY, g.twz, false);
-    vb = (jres == b2) ? free1 : b2;
-  } else {
-    vb = b0; dres = b1; jres = b2;
-  }
-
-  // per-mode update (a7), potential from charge (a2), pad-layer partial sums (a3, fp64)
-  double2 acc[kMaxLayers];
-#pragma unroll
-  for (int l = 0; l < kMaxLayers; ++l) acc[l] = make_double2(0.0, 0.0);
-  const int ty = tid % TY;          // blockDim = 32*TY, so ty is fixed per thread
-  const int ky = ky0 + ty;
-  const double kxd = g.kxd[kx], kyd = g.kyd[ky];
-  const bool ret_x = (kx != nx / 2);
-  for (int t = tid; t < nelem; t += bd) {
-    const int kz = t / TY;
-    const size_t gi = ((size_t)kx * nz + kz) * y2 + ky;
-    const bool ret = ret_x && (kz != nz / 2);
-    const double kzd = g.kzd[kz];
-    double2 r = g.rhat[gi];
-    if (APPLY_J) {
-      const float2 D = dres[t], J = jres[t];
-      const float kzf = (float)kzd;
-      r.x -= (double)(D.x - kzf * J.y);
-      r.y -= (double)(D.y + kzf * J.x);
-      if (!ret) r = make_double2(0.0, 0.0);
-      g.rhat[gi] = r;
-    }
-    double2 src = r;
-    if (DELTA) {
-      const double2 p = g.rhat_prev[gi];
-      src.x -= p.x; src.y -= p.y;
-      g.rhat_prev[gi] = r;
-    }
-    const double k2 = kxd * kxd + kyd * kyd + kzd * kzd;
-    const double gg = (ret && k2 > 0.0) ? gd.inv_n / k2 : 0.0;
-    const double2 v = make_double2(src.x * gg, src.y * gg);
-    vb[t] = make_float2((float)v.x, (float)v.y);
-    dres[t] = make_float2((float)(kzd * v.y), (float)(-kzd * v.x));   // -i kz V^
-#pragma unroll
-    for (int l = 0; l < kMaxLayers; ++l) {
-      if (l < L) {
-        double2 w = g.twzd[(int)(((long long)kz * g.layers[l]) % nz)];
-        w.y = -w.y;                                                    // e^{+i kz z_l}
-        const double2 p = dmul(v, w);
-        acc[l].x += p.x; acc[l].y += p.y;
-      }
-    }
-  }
-#pragma unroll
-  for (int l = 0; l < kMaxLayers; ++l)
-    if (l < L) red[(l * TY + ty) * 32 + tid / TY] = acc[l];
-  __syncthreads();
-  if (tid < L * TY) {
-    double2 s = make_double2(0.0, 0.0);
-    for (int i = 0; i < 32; ++i) { const double2 p = red[tid * 32 + i]; s.x += p.x; s.y += p.y; }
-    pl[tid] = s;
-  }
-  __syncthreads();
-  // contribution of this CTA's (kx, ky tile) modes to the potential at every pad node
-  double* part = (emit ? g.part_e : g.part) + (size_t)blockIdx.x * B;
-  for (int b = tid; b < B; b += bd) {
-    const int l = g.pad_layer[b], x = g.pad_x[b], y = g.pad_y[b];
-    double2 wx = g.twxd[(int)(((long long)kx * x) % nx)];
-    wx.y = -wx.y;
-    double val = 0.0;
-    for (int j = 0; j < TY; ++j) {
-      double2 wy = g.twyd[(int)(((long long)(ky0 + j) * y) % gd.ny)];
-      wy.y = -wy.y;
-      const double2 p = dmul(pl[l * TY + j], dmul(wx, wy));
-      val += ((ky0 + j) == 0 ? 1.0 : 2.0) * p.x;
-    }
-    part[b] = val;
-  }
-  // inverse z transforms (a5, z part)
-  float2* vres = wt::fft_lines<float2>(vb, jres, nz, TY, 1, TY, g.twz, true);
-  float2* fr = (vres == vb) ? jres : vb;
-  for (int t = tid; t < nelem; t += bd) {
-    const int z = t / TY, tyy = t - z * TY;
-    mV[slab + (size_t)z * y2 + tyy] = vres[t];
-  }
-  float2* eres = wt::fft_lines<float2>(dres, fr, nz, TY, 1, TY, g.twz, true);
-  for (int t = tid; t < nelem; t += bd) {
-    const int z = t / TY, tyy = t - z * TY;
-    mE[slab + (size_t)z * y2 + tyy] = eres[t];
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// boundary adjust (a3): rhs, Q' = Ainv rhs, spectrum of the point charges (a4)
-// ------------------------------------------------------------------------------------------------
-// one warp per pad: rhs[b] = flag*V_pad[b] - sum over tiles of the partial potentials (fixed order)
-__global__ void __launch_bounds__(256) k_rhs(GridDev gd, const GeomDev* __restrict__ geoms, int substep, int emit, double flag) {
-  const GeomDev& g = geoms[blockIdx.y];
-  if (substep >= g.n_sub) return;
-  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  if (warp >= g.B) return;
-  const double* part = emit ? g.part_e : g.part;
-  double s = 0.0;
-  for (int c = lane; c < gd.n_tiles; c += 32) s += part[(size_t)c * g.B + warp];
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-  if (lane == 0) g.rhs[warp] = flag * g.pad_pot[warp] - s;
-}
-
-// one warp per row of Ainv
-__global__ void __launch_bounds__(256) k_matvec(const GeomDev* __restrict__ geoms, int substep) {
-  const GeomDev& g = geoms[blockIdx.y];
-  if (substep >= g.n_sub) return;
-  const int warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5, lane = threadIdx.x & 31;
-  if (warp >= g.B) return;
-  const double* row = g.ainv + (size_t)warp * g.B;
-  double s = 0.0;
-  for (int j = lane; j < g.B; j += 32) s += row[j] * g.rhs[j];
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-  if (lane == 0) g.q[warp] = s;
-}
-
-// one thread per (layer, kx, ky): Q^_l = (1/N) sum_{b in l} Q'_b e^{-i(kx x_b + ky y_b)}
-__global__ void __launch_bounds__(256) k_inject(GridDev gd, const GeomDev* __restrict__ geoms, int substep) {
-  const GeomDev& g = geoms[blockIdx.z];
-  if (substep >= g.n_sub) return;
-  const int l = blockIdx.y;
-  if (l >= g.L) return;
-  const int m = blockIdx.x * blockDim.x + threadIdx.x;
-  const int nmodes = gd.nx * gd.y2;
-  __shared__ int sx[256], sy[256];
-  __shared__ double sq[256];
-  const int kx = m / gd.y2, ky = m - kx * gd.y2;
-  double2 acc = make_double2(0.0, 0.0);
-  const int beg = g.layer_off[l], end = g.layer_off[l + 1];
-  for (int c0 = beg; c0 < end; c0 += 256) {
-    const int n = min(256, end - c0);
-    __syncthreads();
-    if ((int)threadIdx.x < n) {
-      const int b = g.layer_idx[c0 + threadIdx.x];
-      sx[threadIdx.x] = g.pad_x[b]; sy[threadIdx.x] = g.pad_y[b]; sq[threadIdx.x] = g.q[b];
-    }
-    __syncthreads();
-    if (m < nmodes) {
-      for (int i = 0; i < n; ++i) {
-        const double2 w = dmul(g.twxd[(int)(((long long)kx * sx[i]) % gd.nx)], g.twyd[(int)(((long long)ky * sy[i]) % gd.ny)]);
-        acc.x += sq[i] * w.x; acc.y += sq[i] * w.y;
-      }
-    }
-  }
-  if (m < nmodes) {
-    if (kx == gd.nx / 2) acc = make_double2(0.0, 0.0);
-    g.qh[(size_t)l * nmodes + m] = make_float2((float)(acc.x * gd.inv_n), (float)(acc.y * gd.inv_n));
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// k_plane: xy-plane transforms.  grid (nz, n_geoms), block 256.
-// Shared memory: three buffers of (nx/2)*(ny+1) float2 used either as a half-spectrum plane
-// [kx][ky] (row stride y2) or as nx/2 complex lines of length ny, each packing the two real
-// x-rows 2p (real part) and 2p+1 (imaginary part), line stride ny+1 (odd: conflict free).
-// ------------------------------------------------------------------------------------------------
-template <bool EMIT>
-__global__ void __launch_bounds__(256) k_plane(GridDev gd, const GeomDev* __restrict__ geoms, int substep, int slot) {
-  const GeomDev& g = geoms[blockIdx.y];
-  if (substep >= g.n_sub) return;
-  const int nx = gd.nx, ny = gd.ny, nz = gd.nz, y2 = gd.y2;
-  const int z = blockIdx.x;
-  const int tid = threadIdx.x, bd = blockDim.x;
-  const int nyp = ny + 1, hx = nx / 2;
-  const int nspec = nx * y2, nline = hx * ny;
-  const int bufsz = hx * nyp;
-  extern __shared__ __align__(16) unsigned char smraw[];
-  float2* dacc = reinterpret_cast<float2*>(smraw);
-  float2* w1 = dacc + bufsz;
-  float2* w2 = w1 + bufsz;
-  const float2* mV = EMIT ? g.e0 : g.m0;
-  const float2* mE = EMIT ? g.e1 : g.m1;
-  const int L = g.L;
-
-  for (int comp = 0; comp < 3; ++comp) {
-    // (1) E~_comp on the half-spectrum plane, boundary-charge part added (a4)
-    for (int t = tid; t < nspec; t += bd) {
-      const int kx = t / y2, ky = t - kx * y2;
-      const size_t gi = ((size_t)kx * nz + z) * y2 + ky;
-      float2 v = (comp == 2) ? mE[gi] : mV[gi];
-      const float* tab = (comp == 2) ? g.gzt : g.gt;
-      for (int l = 0; l < L; ++l) {
-        int dz = z - g.layers[l];
-        if (dz < 0) dz += nz;
-        const float gv = tab[((size_t)kx * nz + dz) * y2 + ky];
-        const float2 qv = g.qh[(size_t)l * nspec + t];
-        v.x += qv.x * gv; v.y += qv.y * gv;
-      }
-      if (comp < 2) {
-        const float kap = (comp == 0) ? (float)g.kxd[kx] : (float)g.kyd[ky];
-        v = make_float2(kap * v.y, -kap * v.x);               // -i kappa V~
-      }
-      w1[t] = v;
-    }
-    __syncthreads();
-    // (2) inverse along x: y2 lines of length nx, element stride y2
-    float2* r = wt::fft_lines<float2>(w1, w2, nx, y2, 1, y2, g.twx, true);
-    float2* o = (r == w1) ? w2 : w1;
-    // (3) pack two x-rows into one complex line with the Hermitian completion along y (Nyquist = 0)
-    for (int t = tid; t < nline; t += bd) {
-      const int p = t / ny, k = t - p * ny;
-      float2 zv;
-      if (k < y2) {
-        const float2 a = r[(2 * p) * y2 + k], b = r[(2 * p + 1) * y2 + k];
-        zv = make_float2(a.x - b.y, a.y + b.x);
-      } else if (k == y2) {
-        zv = make_float2(0.f, 0.f);
-      } else {
-        const float2 a = r[(2 * p) * y2 + (ny - k)], b = r[(2 * p + 1) * y2 + (ny - k)];
-        zv = make_float2(a.x + b.y, b.x - a.y);
-      }
-      o[p * nyp + k] = zv;
-    }
-    __syncthreads();
-    // (4) inverse along y: nx/2 lines of length ny
-    float2* e = wt::fft_lines<float2>(o, r, ny, hx, nyp, 1, g.twy, true);
-    float2* f = (e == o) ? r : o;
-    if (EMIT) {
-      // (a8) H[n] = E/dt into the staging slot, component-planar [slot][comp][z][x][y]
-      float* st = g.stage + (((size_t)slot * 3 + comp) * nz + z) * (size_t)(nx * ny);
-      for (int t = tid; t < nline; t += bd) {
-        const int p = t / ny, y = t - p * ny;
-        const float2 v = e[p * nyp + y];
-        st[(2 * p) * ny + y] = v.x * g.inv_dt;
-        st[(2 * p + 1) * ny + y] = v.y * g.inv_dt;
-      }
-      __syncthreads();
-      continue;
-    }
-    // (5) conduction current J = (s dt_int) E, nodewise (a6, R17)
-    {
-      const uint8_t* sid = g.sig_id + (size_t)z * nx * ny;
-      for (int t = tid; t < nline; t += bd) {
-        const int p = t / ny, y = t - p * ny;
-        float2 v = e[p * nyp + y];
-        v.x *= g.sdt[sid[(2 * p) * ny + y]];
-        v.y *= g.sdt[sid[(2 * p + 1) * ny + y]];
-        e[p * nyp + y] = v;
-      }
-    }
-    __syncthreads();
-    // (6) forward along y
-    float2* jf = wt::fft_lines<float2>(e, f, ny, hx, nyp, 1, g.twy, false);
-    float2* jo = (jf == e) ? f : e;
-    // (7) unpack the two real rows' half spectra
-    for (int t = tid; t < hx * y2; t += bd) {
-      const int p = t / y2, k = t - p * y2;
-      const float2 zk = jf[p * nyp + k];
-      const float2 zm = jf[p * nyp + (k == 0 ? 0 : ny - k)];
-      jo[(2 * p) * y2 + k] = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
-      jo[(2 * p + 1) * y2 + k] = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
-    }
-    __syncthreads();
-    // (8) forward along x
-    float2* jt = wt::fft_lines<float2>(jo, jf, nx, y2, 1, y2, g.twx, false);
-    // (9) D~ = i kx J~x + i ky J~y ; J~z goes out as it is
-    for (int t = tid; t < nspec; t += bd) {
-      const int kx = t / y2, ky = t - kx * y2;
-      const float2 j = jt[t];
-      if (comp == 0) {
-        const float kap = (float)g.kxd[kx];
-        dacc[t] = make_float2(-kap * j.y, kap * j.x);
-      } else if (comp == 1) {
-        const float kap = (float)g.kyd[ky];
-        float2 d = dacc[t];
-        d.x -= kap * j.y; d.y += kap * j.x;
-        dacc[t] = d;
-      } else {
-        const size_t gi = ((size_t)kx * nz + z) * y2 + ky;
-        g.m1[gi] = j;
-        g.m0[gi] = dacc[t];
-      }
-    }
-    __syncthreads();
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// k_transpose: staging [slot][comp][z][x][y] -> H[((x*ny+y)*nz+z)*nt + t][comp] for t0 <= t < t0+cnt.
-// grid (nz*nx, n_geoms), block 256; dynamic smem cnt*3*ny floats.
-// ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_transpose(GridDev gd, const GeomDev* __restrict__ geoms, int t0, int cnt) {
-  const GeomDev& g = geoms[blockIdx.y];
-  const int nx = gd.nx, ny = gd.ny, nz = gd.nz, nt = gd.nt;
-  const int z = blockIdx.x / nx, x = blockIdx.x - z * nx;
-  extern __shared__ float tile[];   // [cnt*3][ny]
-  const int rows = cnt * 3;
-  for (int t = threadIdx.x; t < rows * ny; t += blockDim.x) {
-    const int j = t / ny, y = t - j * ny;          // j = slot*3 + comp
-    tile[t] = g.stage[(((size_t)j * nz + z) * nx + x) * ny + y];
-  }
-  __syncthreads();
-  for (int t = threadIdx.x; t < rows * ny; t += blockDim.x) {
-    const int y = t / rows, j = t - y * rows;
-    g.H[((((size_t)x * ny + y) * nz + z) * nt + t0) * 3 + j] = tile[j * ny + y];
-  }
-}
-
-__global__ void k_zero(double2* p, size_t n) {
-  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < n) p[i] = make_double2(0.0, 0.0);
-}
-
-// ------------------------------------------------------------------------------------------------
-// host side
-// ------------------------------------------------------------------------------------------------
 inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
 int pick_ty(int y2) {
@@ -421,11 +47,47 @@ int pick_ty(int y2) {
   return 1;
 }
 
+bool env_flag(const char* name) {
+  const char* v = std::getenv(name);
+  return v && v[0] && v[0] != '0';
+}
+
+// pads of one geometry grouped by (layer, x)
+struct PadGroups {
+  std::vector<int> grp_x, grp_layer, grp_off, grp_pad, layer_goff, pad_y;
+  int max_per_layer = 0;
+};
+
+PadGroups make_groups(const wt_geometry* g) {
+  PadGroups o;
+  const int B = (int)g->pad_pot.size(), L = (int)g->layers.size();
+  std::map<std::pair<int, int>, std::vector<int>> m;
+  o.pad_y.resize(B);
+  for (int b = 0; b < B; ++b) {
+    m[{g->pad_layer[b], g->pad_nodes[3 * b]}].push_back(b);
+    o.pad_y[b] = g->pad_nodes[3 * b + 1];
+  }
+  o.layer_goff.assign(L + 1, 0);
+  o.grp_off.push_back(0);
+  for (auto& kv : m) {
+    o.grp_layer.push_back(kv.first.first);
+    o.grp_x.push_back(kv.first.second);
+    for (int b : kv.second) o.grp_pad.push_back(b);
+    o.grp_off.push_back((int)o.grp_pad.size());
+    o.layer_goff[kv.first.first + 1]++;
+  }
+  for (int l = 0; l < L; ++l) {
+    o.max_per_layer = std::max(o.max_per_layer, o.layer_goff[l + 1]);
+    o.layer_goff[l + 1] += o.layer_goff[l];
+  }
+  return o;
+}
+
 // Offsets of one geometry's region inside the workspace (static tables, then state).
 struct Layout {
-  size_t sig_id, sdt, gt, gzt, ainv, pad_x, pad_y, pad_layer, pad_pot, layer_off, layer_idx;
-  size_t kxd, kyd, kzd, twx, twy, twz, twxd, twyd, twzd;
-  size_t rhat, rhat_prev, m0, m1, e0, e1, part, part_e, rhs, q, qh, stage;
+  size_t sig_id, sig_t, sdt, gt, gzt, ainv, pad_pot, pad_y, grp_x, grp_layer, grp_off, grp_pad, layer_goff;
+  size_t kxd, kyd, kzd, kxf, kyf, kzf, twx, twy, twz, twxd, twyd, twzd;
+  size_t rhat, rhat_prev, m0, m1, e0, e1, pl, pl_e, rhs, q, qh, stage;
   size_t total;
 };
 
@@ -434,30 +96,24 @@ Layout make_layout(const wt_geometry* g) {
   const size_t nx = g->nx, ny = g->ny, nz = g->nz, y2 = ny / 2;
   const size_t N = nx * ny * nz, half = nx * nz * y2;
   const size_t B = g->pad_pot.size(), L = g->layers.size();
-  const size_t tiles = nx * (y2 / pick_ty((int)y2));
   size_t p = 0;
   auto take = [&](size_t bytes) { size_t at = p; p = align_up(p + bytes); return at; };
-  o.sig_id = take(N); o.sdt = take(256 * 4); o.gt = take(half * 4); o.gzt = take(half * 4);
-  o.ainv = take(B * B * 8); o.pad_x = take(B * 4); o.pad_y = take(B * 4); o.pad_layer = take(B * 4);
-  o.pad_pot = take(B * 8); o.layer_off = take((L + 1) * 4); o.layer_idx = take(B * 4);
+  o.sig_id = take(N); o.sig_t = take(N); o.sdt = take(256 * 4); o.gt = take(half * 4); o.gzt = take(half * 4);
+  o.ainv = take(B * B * 8); o.pad_pot = take(B * 8); o.pad_y = take(B * 4);
+  o.grp_x = take(B * 4); o.grp_layer = take(B * 4); o.grp_off = take((B + 1) * 4); o.grp_pad = take(B * 4);
+  o.layer_goff = take((L + 1) * 4);
   o.kxd = take(nx * 8); o.kyd = take(y2 * 8); o.kzd = take(nz * 8);
+  o.kxf = take(nx * 4); o.kyf = take(y2 * 4); o.kzf = take(nz * 4);
   o.twx = take(nx * 8); o.twy = take(ny * 8); o.twz = take(nz * 8);
   o.twxd = take(nx * 16); o.twyd = take(ny * 16); o.twzd = take(nz * 16);
   o.rhat = take(half * 16); o.rhat_prev = take(half * 16);
   o.m0 = take(half * 8); o.m1 = take(half * 8); o.e0 = take(half * 8); o.e1 = take(half * 8);
-  o.part = take(tiles * B * 8); o.part_e = take(tiles * B * 8);
+  o.pl = take(L * nx * y2 * 16); o.pl_e = take(L * nx * y2 * 16);
   o.rhs = take(B * 8); o.q = take(B * 8); o.qh = take(L * nx * y2 * 8);
   o.stage = take((size_t)kStageSlots * 3 * N * 4);
   o.total = p;
   return o;
 }
-
-size_t spectral_smem(const wt_geometry* g) {
-  const int y2 = g->ny / 2, ty = pick_ty(y2);
-  const size_t L = g->layers.size();
-  return (size_t)3 * g->nz * ty * 8 + (L * ty * 32 + L * ty) * 16;
-}
-size_t plane_smem(const wt_geometry* g) { return (size_t)3 * (g->nx / 2) * (g->ny + 1) * 8; }
 
 template <typename T>
 cudaError_t upload(char* base, size_t off, const std::vector<T>& v, cudaStream_t st) {
@@ -474,10 +130,80 @@ cudaError_t upload(char* base, size_t off, const std::vector<T>& v, cudaStream_t
     }                                                                                         \
   } while (0)
 
+// ---- kernel selection ---------------------------------------------------------------------------
+using PlaneFn = void (*)(GridDev, const GeomDev*, int);
+using LineFn = void (*)(GridDev, const GeomDev*, int, int);
+
+struct Plan {
+  PlaneFn plane_step = nullptr, plane_emit = nullptr;
+  dim3 plane_block;
+  size_t plane_smem = 0;
+  bool plane_fast = false;     // staging layout [z][y][x] instead of [z][x][y]
+  LineFn line_step = nullptr, line_init = nullptr, line_delta = nullptr;   // <J>, <>, <DELTA>
+  dim3 line_grid, line_block;
+  size_t line_smem = 0;
+  bool line_fast = false;
+  int ty = 1;
+};
+
+template <int N, int E, int CP>
+void set_plane(Plan& p) {
+  p.plane_step = k_plane_fast<N, E, CP, false>;
+  p.plane_emit = k_plane_fast<N, E, CP, true>;
+  p.plane_block = dim3(N * N / (2 * E));
+  p.plane_smem = (size_t)2 * CP * PlaneCfg<N>::BUF * sizeof(float2);
+  p.plane_fast = true;
+}
+
+template <int NZ, int E, int TYL>
+void set_line(Plan& p, int nx, int y2, int L, int n_geoms) {
+  using C = PencilCfg<NZ, E, TYL>;
+  p.line_step = k_pencil<NZ, E, TYL, true, false>;
+  p.line_init = k_pencil<NZ, E, TYL, false, false>;
+  p.line_delta = k_pencil<NZ, E, TYL, false, true>;
+  p.line_grid = dim3(nx * (y2 / TYL), n_geoms);
+  p.line_block = dim3(C::THREADS);
+  p.line_smem = (size_t)2 * C::FIELD * sizeof(float2) + (size_t)std::max(1, L) * TYL * C::T * sizeof(double2);
+  p.line_fast = true;
+  p.ty = TYL;
+}
+
+Plan make_plan(int nx, int ny, int nz, int L, int n_geoms, bool force_generic) {
+  Plan p;
+  const int y2 = ny / 2;
+  if (!force_generic && nx == ny) {
+    if (nx == 32) set_plane<32, 8, 3>(p);
+    else if (nx == 64) set_plane<64, 8, 3>(p);
+    else if (nx == 128) set_plane<128, 16, 1>(p);
+  }
+  if (!p.plane_fast) {
+    p.plane_step = k_plane<false>;
+    p.plane_emit = k_plane<true>;
+    p.plane_block = dim3(256);
+    p.plane_smem = (size_t)3 * (nx / 2) * (ny + 1) * sizeof(float2);
+  }
+  if (!force_generic) {
+    if (nz == 256 && y2 % 8 == 0) set_line<256, 16, 8>(p, nx, y2, L, n_geoms);
+    else if (nz == 128 && y2 % 16 == 0) set_line<128, 16, 16>(p, nx, y2, L, n_geoms);
+    else if (nz == 64 && y2 % 16 == 0) set_line<64, 8, 16>(p, nx, y2, L, n_geoms);
+    else if (nz == 32 && y2 % 16 == 0) set_line<32, 8, 16>(p, nx, y2, L, n_geoms);
+  }
+  if (!p.line_fast) {
+    p.ty = pick_ty(y2);
+    p.line_step = k_spectral<true, false>;
+    p.line_init = k_spectral<false, false>;
+    p.line_delta = k_spectral<false, true>;
+    p.line_grid = dim3(nx * (y2 / p.ty), n_geoms);
+    p.line_block = dim3(32 * p.ty);
+    p.line_smem = (size_t)3 * nz * p.ty * sizeof(float2) + (size_t)std::max(1, L) * p.ty * 32 * sizeof(double2);
+  }
+  return p;
+}
+
 }  // namespace
 
-// bytes wt_solve_H needs for this geometry (its region + one descriptor slot)
-size_t wt_solve_workspace_bytes(const wt_geometry* g) { return make_layout(g).total + align_up(sizeof(GeomDev)); }
+// bytes wt_solve_H needs for this geometry (its region + one descriptor slot + the step counter)
+size_t wt_solve_workspace_bytes(const wt_geometry* g) { return make_layout(g).total + align_up(sizeof(GeomDev)) + 256; }
 
 extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* H_dev, size_t H_bytes_each,
                           void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
@@ -499,22 +225,34 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     regions += make_layout(g).total;
     max_sub = std::max(max_sub, g->n_sub);
   }
-  const size_t need = regions + align_up((size_t)n_geoms * sizeof(GeomDev));
+  const size_t need = regions + align_up((size_t)n_geoms * sizeof(GeomDev)) + 256;
   const size_t hbytes = (size_t)g0->nx * g0->ny * g0->nz * g0->nt * 12;
   if (H_bytes_each < hbytes) { wt_set_error("wt_solve_H: H_bytes_each too small"); return WT_EINVAL; }
   if (((uintptr_t)workspace_dev) % 256 != 0) { wt_set_error("wt_solve_H: workspace not 256-byte aligned"); return WT_EINVAL; }
   if (workspace_bytes < need) { wt_set_error("wt_solve_H: workspace too small, need " + std::to_string(need)); return WT_ENOMEM; }
-  size_t sm_spec = 0;
-  const size_t sm_plane = plane_smem(g0);
-  for (int i = 0; i < n_geoms; ++i) sm_spec = std::max(sm_spec, spectral_smem(geoms[i]));
-  if (sm_spec > 227 * 1024 || sm_plane > 227 * 1024) {
-    wt_set_error("wt_solve_H: grid too large for the shared-memory tiles (nx*ny <= 128*128)"); return WT_EINVAL;
-  }
+
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int nx = g0->nx, ny = g0->ny, nz = g0->nz, y2 = ny / 2, nt = g0->nt;
-  const int TY = pick_ty(y2);
+  int maxB = 0, maxL = 0, maxG = 0, maxGL = 0;
+  std::vector<PadGroups> groups(n_geoms);
+  for (int i = 0; i < n_geoms; ++i) {
+    groups[i] = make_groups(geoms[i]);
+    maxB = std::max(maxB, (int)geoms[i]->pad_pot.size());
+    maxL = std::max(maxL, (int)geoms[i]->layers.size());
+    maxG = std::max(maxG, (int)groups[i].grp_x.size());
+    maxGL = std::max(maxGL, groups[i].max_per_layer);
+  }
+  const Plan plan = make_plan(nx, ny, nz, maxL, n_geoms, env_flag("WTIDE_GENERIC"));
+  const size_t sm_padpot = (size_t)(kPadChunks + 1) * y2 * sizeof(double2);
+  const size_t sm_inject = (size_t)std::max(1, maxGL) * y2 * sizeof(double2);
+  const size_t sm_tr = (size_t)kStageSlots * 3 * std::max(nx, ny) * sizeof(float);
+  const size_t kMaxSmem = 227 * 1024;
+  if (plan.plane_smem > kMaxSmem || plan.line_smem > kMaxSmem || sm_padpot > kMaxSmem || sm_inject > kMaxSmem || sm_tr > kMaxSmem) {
+    wt_set_error("wt_solve_H: grid too large for the shared-memory tiles (nx*ny <= 128*128, nz <= 1024)"); return WT_EINVAL;
+  }
+
   GridDev gd;
-  gd.nx = nx; gd.ny = ny; gd.nz = nz; gd.y2 = y2; gd.nt = nt; gd.ty = TY; gd.n_tiles = nx * (y2 / TY);
+  gd.nx = nx; gd.ny = ny; gd.nz = nz; gd.y2 = y2; gd.nt = nt; gd.ty = plan.ty; gd.n_tiles = nx * (y2 / plan.ty);
   gd.inv_n = 1.0 / ((double)nx * ny * nz);
 
   // twiddles e^{-2 pi i k/n} (fp64 on the host)
@@ -534,106 +272,143 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   std::vector<GeomDev> hd(n_geoms);
   char* base = (char*)workspace_dev;
   size_t off = 0;
-  int maxB = 0, maxL = 0;
+  std::vector<std::vector<uint8_t>> sig_t(n_geoms);
+  std::vector<std::vector<float>> kf(3 * n_geoms);
   for (int i = 0; i < n_geoms; ++i) {
     const wt_geometry* g = geoms[i];
     const Layout lo = make_layout(g);
+    const PadGroups& pg = groups[i];
     char* b = base + off;
     const int B = (int)g->pad_pot.size(), L = (int)g->layers.size();
-    maxB = std::max(maxB, B); maxL = std::max(maxL, L);
-    std::vector<int> px(B), py(B), loff(L + 1, 0), lidx(B);
-    for (int k = 0; k < B; ++k) { px[k] = g->pad_nodes[3 * k]; py[k] = g->pad_nodes[3 * k + 1]; }
-    for (int k = 0; k < B; ++k) loff[g->pad_layer[k] + 1]++;
-    for (int l = 0; l < L; ++l) loff[l + 1] += loff[l];
-    {
-      std::vector<int> cur(loff.begin(), loff.end() - 1);
-      for (int k = 0; k < B; ++k) lidx[cur[g->pad_layer[k]]++] = k;
-    }
-    CK(upload(b, lo.sig_id, g->sig_id, st)); CK(upload(b, lo.sdt, g->sdt, st));
+    sig_t[i].resize(g->sig_id.size());
+    for (int z = 0; z < nz; ++z)
+      for (int x = 0; x < nx; ++x)
+        for (int y = 0; y < ny; ++y) sig_t[i][((size_t)z * ny + y) * nx + x] = g->sig_id[((size_t)z * nx + x) * ny + y];
+    std::vector<float>&kxf = kf[3 * i], &kyf = kf[3 * i + 1], &kzf = kf[3 * i + 2];
+    kxf.assign(g->kx.begin(), g->kx.end()); kyf.assign(g->ky.begin(), g->ky.end()); kzf.assign(g->kz.begin(), g->kz.end());
+    CK(upload(b, lo.sig_id, g->sig_id, st)); CK(upload(b, lo.sig_t, sig_t[i], st)); CK(upload(b, lo.sdt, g->sdt, st));
     CK(upload(b, lo.gt, g->gt, st)); CK(upload(b, lo.gzt, g->gzt, st));
-    CK(upload(b, lo.ainv, g->ainv, st));
-    CK(upload(b, lo.pad_x, px, st)); CK(upload(b, lo.pad_y, py, st));
-    CK(upload(b, lo.pad_layer, g->pad_layer, st)); CK(upload(b, lo.pad_pot, g->pad_pot, st));
-    CK(upload(b, lo.layer_off, loff, st)); CK(upload(b, lo.layer_idx, lidx, st));
+    CK(upload(b, lo.ainv, g->ainv, st)); CK(upload(b, lo.pad_pot, g->pad_pot, st)); CK(upload(b, lo.pad_y, pg.pad_y, st));
+    CK(upload(b, lo.grp_x, pg.grp_x, st)); CK(upload(b, lo.grp_layer, pg.grp_layer, st));
+    CK(upload(b, lo.grp_off, pg.grp_off, st)); CK(upload(b, lo.grp_pad, pg.grp_pad, st));
+    CK(upload(b, lo.layer_goff, pg.layer_goff, st));
     CK(upload(b, lo.kxd, g->kx, st)); CK(upload(b, lo.kyd, g->ky, st)); CK(upload(b, lo.kzd, g->kz, st));
+    CK(upload(b, lo.kxf, kxf, st)); CK(upload(b, lo.kyf, kyf, st)); CK(upload(b, lo.kzf, kzf, st));
     CK(upload(b, lo.twx, twx, st)); CK(upload(b, lo.twy, twy, st)); CK(upload(b, lo.twz, twz, st));
     CK(upload(b, lo.twxd, twxd, st)); CK(upload(b, lo.twyd, twyd, st)); CK(upload(b, lo.twzd, twzd, st));
     GeomDev& d = hd[i];
-    d.sig_id = (const uint8_t*)(b + lo.sig_id); d.sdt = (const float*)(b + lo.sdt);
+    d.sig_id = (const uint8_t*)(b + lo.sig_id); d.sig_t = (const uint8_t*)(b + lo.sig_t); d.sdt = (const float*)(b + lo.sdt);
     d.gt = (const float*)(b + lo.gt); d.gzt = (const float*)(b + lo.gzt);
-    d.ainv = (const double*)(b + lo.ainv);
-    d.pad_x = (const int*)(b + lo.pad_x); d.pad_y = (const int*)(b + lo.pad_y);
-    d.pad_layer = (const int*)(b + lo.pad_layer); d.pad_pot = (const double*)(b + lo.pad_pot);
-    d.layer_off = (const int*)(b + lo.layer_off); d.layer_idx = (const int*)(b + lo.layer_idx);
+    d.ainv = (const double*)(b + lo.ainv); d.pad_pot = (const double*)(b + lo.pad_pot); d.pad_y = (const int*)(b + lo.pad_y);
+    d.grp_x = (const int*)(b + lo.grp_x); d.grp_layer = (const int*)(b + lo.grp_layer);
+    d.grp_off = (const int*)(b + lo.grp_off); d.grp_pad = (const int*)(b + lo.grp_pad);
+    d.layer_goff = (const int*)(b + lo.layer_goff);
     d.kxd = (const double*)(b + lo.kxd); d.kyd = (const double*)(b + lo.kyd); d.kzd = (const double*)(b + lo.kzd);
+    d.kxf = (const float*)(b + lo.kxf); d.kyf = (const float*)(b + lo.kyf); d.kzf = (const float*)(b + lo.kzf);
     d.twx = (const float2*)(b + lo.twx); d.twy = (const float2*)(b + lo.twy); d.twz = (const float2*)(b + lo.twz);
     d.twxd = (const double2*)(b + lo.twxd); d.twyd = (const double2*)(b + lo.twyd); d.twzd = (const double2*)(b + lo.twzd);
     d.rhat = (double2*)(b + lo.rhat); d.rhat_prev = (double2*)(b + lo.rhat_prev);
     d.m0 = (float2*)(b + lo.m0); d.m1 = (float2*)(b + lo.m1); d.e0 = (float2*)(b + lo.e0); d.e1 = (float2*)(b + lo.e1);
-    d.part = (double*)(b + lo.part); d.part_e = (double*)(b + lo.part_e);
+    d.pl = (double2*)(b + lo.pl); d.pl_e = (double2*)(b + lo.pl_e);
     d.rhs = (double*)(b + lo.rhs); d.q = (double*)(b + lo.q); d.qh = (float2*)(b + lo.qh);
     d.stage = (float*)(b + lo.stage);
     d.H = H_dev[i];
     for (int l = 0; l < kMaxLayers; ++l) d.layers[l] = (l < L) ? g->layers[l] : 0;
-    d.B = B; d.L = L; d.n_sub = g->n_sub; d.inv_dt = (float)(1.0 / g->dt);
+    d.B = B; d.L = L; d.G = (int)pg.grp_x.size(); d.n_sub = g->n_sub; d.inv_dt = (float)(1.0 / g->dt);
     off += lo.total;
   }
   GeomDev* dgeoms = (GeomDev*)(base + off);
   CK(cudaMemcpyAsync(dgeoms, hd.data(), (size_t)n_geoms * sizeof(GeomDev), cudaMemcpyHostToDevice, st));
+  int* dstep = (int*)(base + off + align_up((size_t)n_geoms * sizeof(GeomDev)));
+  gd.step = dstep;
+  CK(cudaMemsetAsync(dstep, 0, sizeof(int), st));
+  // the uploads above read pageable host vectors: cudaMemcpyAsync has staged them before it returns
 
   // ---- launch configuration -------------------------------------------------------------------
-  CK(cudaFuncSetAttribute(k_spectral<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_spec));
-  CK(cudaFuncSetAttribute(k_spectral<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_spec));
-  CK(cudaFuncSetAttribute(k_spectral<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_spec));
-  CK(cudaFuncSetAttribute(k_plane<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_plane));
-  CK(cudaFuncSetAttribute(k_plane<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm_plane));
-  const dim3 g_spec(gd.n_tiles, n_geoms), b_spec(32 * TY);
+  auto set_smem = [&](const void* fn, size_t bytes) -> cudaError_t {
+    return cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  };
+  CK(set_smem((const void*)plan.plane_step, plan.plane_smem)); CK(set_smem((const void*)plan.plane_emit, plan.plane_smem));
+  CK(set_smem((const void*)plan.line_step, plan.line_smem)); CK(set_smem((const void*)plan.line_init, plan.line_smem));
+  CK(set_smem((const void*)plan.line_delta, plan.line_smem));
+  CK(set_smem((const void*)k_padpot, sm_padpot)); CK(set_smem((const void*)k_inject, sm_inject));
+  CK(set_smem((const void*)k_transpose<false>, sm_tr)); CK(set_smem((const void*)k_transpose<true>, sm_tr));
   const dim3 g_plane(nz, n_geoms);
-  const dim3 g_warpB((maxB * 32 + 255) / 256, n_geoms);
-  const dim3 g_inj((nx * y2 + 255) / 256, maxL, n_geoms);
-  const dim3 g_tr(nz * nx, n_geoms);
+  const dim3 g_pot(std::max(1, maxG), n_geoms);
+  const dim3 g_mv((maxB * 32 + 255) / 256, n_geoms);
+  const dim3 g_inj((nx + kInjKx - 1) / kInjKx, std::max(1, maxL), n_geoms);
+  const dim3 g_tr(plan.plane_fast ? nz * ny : nz * nx, n_geoms);
   const size_t half = (size_t)nx * nz * y2;
 
+  long long launches = 0;
   auto boundary = [&](int s, int emit, double flag) {
     if (maxB == 0) return;
-    g_wt_launches += 3;
-    k_rhs<<<g_warpB, 256, 0, st>>>(gd, dgeoms, s, emit, flag);
-    k_matvec<<<g_warpB, 256, 0, st>>>(dgeoms, s);
-    k_inject<<<g_inj, 256, 0, st>>>(gd, dgeoms, s);
+    launches += 3;
+    k_padpot<<<g_pot, 256, sm_padpot, st>>>(gd, dgeoms, s, emit, flag);
+    k_matvec<<<g_mv, 256, 0, st>>>(dgeoms, s);
+    k_inject<<<g_inj, 256, sm_inject, st>>>(gd, dgeoms, s);
   };
-  auto emit_step = [&](int n) {
+  auto emit_step = [&](bool first) {
     // H[n] from the increment of the charge since the previous output step (the prompt response
-    // H[0] from the pads alone: r = 0, pads at v_w)
-    g_wt_launches += 2;
-    if (n == 0) k_spectral<false, false><<<g_spec, b_spec, sm_spec, st>>>(gd, dgeoms, 0, 1);
-    else        k_spectral<false, true><<<g_spec, b_spec, sm_spec, st>>>(gd, dgeoms, 0, 1);
-    boundary(0, 1, n == 0 ? 1.0 : 0.0);
-    k_plane<true><<<g_plane, 256, sm_plane, st>>>(gd, dgeoms, 0, n % kStageSlots);
-    if ((n + 1) % kStageSlots == 0 || n == nt - 1) {
-      const int cnt = n % kStageSlots + 1, t0 = n - cnt + 1;
-      ++g_wt_launches;
-      k_transpose<<<g_tr, 256, (size_t)cnt * 3 * ny * sizeof(float), st>>>(gd, dgeoms, t0, cnt);
-    }
+    // H[0] from the pads alone: r = 0, pads at v_w); n is read from the device counter
+    launches += 4;
+    const LineFn line_emit = first ? plan.line_init : plan.line_delta;
+    line_emit<<<plan.line_grid, plan.line_block, plan.line_smem, st>>>(gd, dgeoms, 0, 1);
+    boundary(0, 1, first ? 1.0 : 0.0);
+    plan.plane_emit<<<g_plane, plan.plane_block, plan.plane_smem, st>>>(gd, dgeoms, 0);
+    if (plan.plane_fast) k_transpose<true><<<g_tr, 256, sm_tr, st>>>(gd, dgeoms);
+    else                 k_transpose<false><<<g_tr, 256, sm_tr, st>>>(gd, dgeoms);
+    k_advance<<<1, 1, 0, st>>>(dstep);
   };
-
-  g_wt_launches += 2 * n_geoms + 1;
-  for (int i = 0; i < n_geoms; ++i) {
-    k_zero<<<(unsigned)((half + 255) / 256), 256, 0, st>>>(hd[i].rhat, half);
-    k_zero<<<(unsigned)((half + 255) / 256), 256, 0, st>>>(hd[i].rhat_prev, half);
-    if (maxL > 0) CK(cudaMemsetAsync(hd[i].qh, 0, (size_t)hd[i].L * nx * y2 * sizeof(float2), st));
-  }
-  emit_step(0);
-  k_spectral<false, false><<<g_spec, b_spec, sm_spec, st>>>(gd, dgeoms, 0, 0);
-  for (int n = 1; n < nt; ++n) {
+  auto output_step = [&]() {
     for (int s = 0; s < max_sub; ++s) {
       boundary(s, 0, 1.0);
-      g_wt_launches += 2;
-      k_plane<false><<<g_plane, 256, sm_plane, st>>>(gd, dgeoms, s, 0);
-      k_spectral<true, false><<<g_spec, b_spec, sm_spec, st>>>(gd, dgeoms, s, 0);
+      launches += 2;
+      plan.plane_step<<<g_plane, plan.plane_block, plan.plane_smem, st>>>(gd, dgeoms, s);
+      plan.line_step<<<plan.line_grid, plan.line_block, plan.line_smem, st>>>(gd, dgeoms, s, 0);
     }
-    emit_step(n);
+    emit_step(false);
+  };
+
+  for (int i = 0; i < n_geoms; ++i) {
+    CK(cudaMemsetAsync(hd[i].rhat, 0, half * sizeof(double2), st));
+    CK(cudaMemsetAsync(hd[i].rhat_prev, 0, half * sizeof(double2), st));
+    if (hd[i].L > 0) CK(cudaMemsetAsync(hd[i].qh, 0, (size_t)hd[i].L * nx * y2 * sizeof(float2), st));
+  }
+  emit_step(true);
+  ++launches;
+  plan.line_init<<<plan.line_grid, plan.line_block, plan.line_smem, st>>>(gd, dgeoms, 0, 0);
+  CK(cudaGetLastError());
+
+  const int n_out = nt - 1;
+  if (n_out >= 2 && !env_flag("WTIDE_NO_GRAPH")) {
+    // one output step captured once, replayed n_out times
+    const long long before = launches;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+    output_step();
+    cudaError_t ec = cudaStreamEndCapture(st, &graph);
+    if (ec != cudaSuccess || !graph) {
+      wt_set_error(std::string("wt_solve_H: stream capture failed: ") + cudaGetErrorString(ec)); return WT_ECUDA;
+    }
+    const long long per_step = launches - before;
+    ec = cudaGraphInstantiate(&exec, graph, 0);
+    if (ec != cudaSuccess) {
+      cudaGraphDestroy(graph);
+      wt_set_error(std::string("wt_solve_H: graph instantiation failed: ") + cudaGetErrorString(ec)); return WT_ECUDA;
+    }
+    for (int n = 0; n < n_out && ec == cudaSuccess; ++n) ec = cudaGraphLaunch(exec, st);
+    launches = before + per_step * n_out;
+    // an executable graph that is in flight is freed asynchronously on completion
+    cudaGraphExecDestroy(exec);
+    cudaGraphDestroy(graph);
+    if (ec != cudaSuccess) { wt_set_error(std::string("wt_solve_H: graph launch failed: ") + cudaGetErrorString(ec)); return WT_ECUDA; }
+  } else {
+    for (int n = 0; n < n_out; ++n) output_step();
   }
   CK(cudaGetLastError());
+  g_wt_launches += launches;
   wt_set_error("");
   return WT_OK;
 }

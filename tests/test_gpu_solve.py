@@ -32,10 +32,22 @@ def _slice_report(h, ref):
     return num / np.maximum(den, 1e-300)
 
 
-@pytest.mark.parametrize("grid,nt", [((32, 32, 32), 8), ((12, 24, 18), 4), ((16, 8, 6), 12)])
-def test_small_tables_match_the_oracle(grid, nt):
-    """Config 0 geometry on its own grid (window of 8 output steps = 280 Euler substeps) and on two
-    ragged grids with radix-3 factors and nx != ny != nz."""
+@pytest.mark.parametrize("grid,nt,env", [
+    ((32, 32, 32), 8, {}),                        # register-FFT plane + z-line kernels
+    ((32, 32, 32), 8, {"WTIDE_GENERIC": "1"}),    # the size-generic kernels on the same grid
+    ((32, 32, 32), 8, {"WTIDE_NO_GRAPH": "1"}),   # direct launches instead of the replayed CUDA graph
+    ((12, 24, 18), 4, {}), ((16, 8, 6), 12, {}),  # ragged grids with radix-3 factors (generic kernels)
+    ((32, 32, 6), 4, {}),                         # register-FFT plane kernel + generic z-line kernel
+    ((16, 16, 256), 4, {}),                       # generic plane kernel + register-FFT z-line kernel (nz = 256)
+    ((64, 64, 4), 4, {}), ((128, 128, 4), 4, {}), # the 64^2 and 128^2 plane kernels
+    ((16, 32, 128), 4, {}),                       # nz = 128 z-line kernel
+])
+def test_small_tables_match_the_oracle(grid, nt, env, monkeypatch):
+    """Config 0 geometry on its own grid (window of 8 output steps = 280 Euler substeps), on ragged
+    grids with radix-3 factors and nx != ny != nz, and on grids that select each size-specialised
+    kernel of solve_fast.cuh."""
+    for k, v in env.items():
+        monkeypatch.setenv(k, v)
     d = reduced_desc(geometry_desc(0), grid=grid, nt=nt)
     _, (h,) = _solve([d])
     ref = wo.solve_H_from_desc(d)
