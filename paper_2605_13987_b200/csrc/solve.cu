@@ -7,11 +7,12 @@
 // live in "mixed space" arrays M[kx][z][ky] (ky >= 0 half spectrum).
 //
 // One Euler substep =
-//   k_padpot   pad potentials of the free charge from pl = V~_rho at the pad layers -> rhs           (a3)
-//   k_matvec   Q' = Ainv rhs: "adjusted, in magnitude, to enforce the boundary conditions"          (a3)
-//   k_inject   spectrum of the boundary point charges per pad layer                                 (a4)
+//   boundary   pad potentials of the free charge from pl = V~_rho at the pad layers -> rhs;           (a3)
+//              Q' = Ainv rhs: "adjusted, in magnitude, to enforce the boundary conditions";          (a3)
+//              spectrum of the boundary point charges per pad layer                                 (a4)
+//              (one cluster launch, or three grid-wide launches for large pad sets)
 //   plane      V~ = V~_rho + sum_l Q^_l * g~ (translated fundamental solution, a4); E~ = -i kappa V~;
-//              inverse xy DFT (a5); J = s dt_int E (a6); forward xy DFT; D~ = i kx J~x + i ky J~y
+//              inverse xy DFT (a5); J = s dt_int E (a6); forward xy DFT; i kx J~x, i ky J~y, J~z
 //   z-line     forward z DFT; r^ -= D^ + i kz J^z (a7, fp64 state); V^ = r^/|kappa|^2 (a2);
 //              pl (fp64); inverse z DFT of V^ and -i kz V^
 // Every n_sub substeps the same kernels run once on the increment r^ - r^_prev with the pads at
@@ -52,9 +53,11 @@ bool env_flag(const char* name) {
   return v && v[0] && v[0] != '0';
 }
 
-// pads of one geometry grouped by (layer, x)
+// pads of one geometry grouped by (layer, x); perm[i] = index (in the handle's pad order) of the
+// i-th pad in group order; the device holds every per-pad array in group order
 struct PadGroups {
-  std::vector<int> grp_x, grp_layer, grp_off, grp_pad, layer_goff, pad_y;
+  std::vector<int> grp_x, grp_layer, grp_off, perm, layer_goff, pad_y;
+  std::vector<double> pad_pot, ainv;
   int max_per_layer = 0;
 };
 
@@ -62,32 +65,34 @@ PadGroups make_groups(const wt_geometry* g) {
   PadGroups o;
   const int B = (int)g->pad_pot.size(), L = (int)g->layers.size();
   std::map<std::pair<int, int>, std::vector<int>> m;
-  o.pad_y.resize(B);
-  for (int b = 0; b < B; ++b) {
-    m[{g->pad_layer[b], g->pad_nodes[3 * b]}].push_back(b);
-    o.pad_y[b] = g->pad_nodes[3 * b + 1];
-  }
+  for (int b = 0; b < B; ++b) m[{g->pad_layer[b], g->pad_nodes[3 * b]}].push_back(b);
   o.layer_goff.assign(L + 1, 0);
   o.grp_off.push_back(0);
   for (auto& kv : m) {
     o.grp_layer.push_back(kv.first.first);
     o.grp_x.push_back(kv.first.second);
-    for (int b : kv.second) o.grp_pad.push_back(b);
-    o.grp_off.push_back((int)o.grp_pad.size());
+    for (int b : kv.second) o.perm.push_back(b);
+    o.grp_off.push_back((int)o.perm.size());
     o.layer_goff[kv.first.first + 1]++;
   }
   for (int l = 0; l < L; ++l) {
     o.max_per_layer = std::max(o.max_per_layer, o.layer_goff[l + 1]);
     o.layer_goff[l + 1] += o.layer_goff[l];
   }
+  o.pad_y.resize(B); o.pad_pot.resize(B); o.ainv.resize((size_t)B * B);
+  for (int i = 0; i < B; ++i) {
+    o.pad_y[i] = g->pad_nodes[3 * o.perm[i] + 1];
+    o.pad_pot[i] = g->pad_pot[o.perm[i]];
+    for (int k = 0; k < B; ++k) o.ainv[(size_t)i * B + k] = g->ainv[(size_t)o.perm[i] * B + o.perm[k]];
+  }
   return o;
 }
 
 // Offsets of one geometry's region inside the workspace (static tables, then state).
 struct Layout {
-  size_t sig_id, sig_t, sdt, gt, gzt, ainv, pad_pot, pad_y, grp_x, grp_layer, grp_off, grp_pad, layer_goff;
+  size_t sig_id, sig_t, sdt, gt, gzt, ainv, pad_pot, pad_y, grp_x, grp_layer, grp_off, layer_goff;
   size_t kxd, kyd, kzd, kxf, kyf, kzf, twx, twy, twz, twxd, twyd, twzd;
-  size_t rhat, rhat_prev, m0, m1, e0, e1, pl, pl_e, rhs, q, qh, stage;
+  size_t rhat, rhat_prev, v0, v1, m0, m1, m2, e0, e1, pl, pl_e, rhs, q, qh, stage;
   size_t total;
 };
 
@@ -100,14 +105,15 @@ Layout make_layout(const wt_geometry* g) {
   auto take = [&](size_t bytes) { size_t at = p; p = align_up(p + bytes); return at; };
   o.sig_id = take(N); o.sig_t = take(N); o.sdt = take(256 * 4); o.gt = take(half * 4); o.gzt = take(half * 4);
   o.ainv = take(B * B * 8); o.pad_pot = take(B * 8); o.pad_y = take(B * 4);
-  o.grp_x = take(B * 4); o.grp_layer = take(B * 4); o.grp_off = take((B + 1) * 4); o.grp_pad = take(B * 4);
+  o.grp_x = take(B * 4); o.grp_layer = take(B * 4); o.grp_off = take((B + 1) * 4);
   o.layer_goff = take((L + 1) * 4);
   o.kxd = take(nx * 8); o.kyd = take(y2 * 8); o.kzd = take(nz * 8);
   o.kxf = take(nx * 4); o.kyf = take(y2 * 4); o.kzf = take(nz * 4);
   o.twx = take(nx * 8); o.twy = take(ny * 8); o.twz = take(nz * 8);
   o.twxd = take(nx * 16); o.twyd = take(ny * 16); o.twzd = take(nz * 16);
   o.rhat = take(half * 16); o.rhat_prev = take(half * 16);
-  o.m0 = take(half * 8); o.m1 = take(half * 8); o.e0 = take(half * 8); o.e1 = take(half * 8);
+  o.v0 = take(half * 8); o.v1 = take(half * 8);
+  o.m0 = take(half * 8); o.m1 = take(half * 8); o.m2 = take(half * 8); o.e0 = take(half * 8); o.e1 = take(half * 8);
   o.pl = take(L * nx * y2 * 16); o.pl_e = take(L * nx * y2 * 16);
   o.rhs = take(B * 8); o.q = take(B * 8); o.qh = take(L * nx * y2 * 8);
   o.stage = take((size_t)kStageSlots * 3 * N * 4);
@@ -131,14 +137,14 @@ cudaError_t upload(char* base, size_t off, const std::vector<T>& v, cudaStream_t
   } while (0)
 
 // ---- kernel selection ---------------------------------------------------------------------------
-using PlaneFn = void (*)(GridDev, const GeomDev*, int);
-using LineFn = void (*)(GridDev, const GeomDev*, int, int);
+using PlaneFn = void (*)(const GeomBatch, GridDev, int);
+using LineFn = void (*)(const GeomBatch, GridDev, int, int);
 
 struct Plan {
   PlaneFn plane_step = nullptr, plane_emit = nullptr;
   dim3 plane_block;
   size_t plane_smem = 0;
-  bool plane_fast = false;     // staging layout [z][y][x] instead of [z][x][y]
+  bool plane_fast = false;     // one CTA per (z, component); staging layout [z][y][x] instead of [z][x][y]
   LineFn line_step = nullptr, line_init = nullptr, line_delta = nullptr;   // <J>, <>, <DELTA>
   dim3 line_grid, line_block;
   size_t line_smem = 0;
@@ -146,54 +152,59 @@ struct Plan {
   int ty = 1;
 };
 
-template <int N, int E, int CP>
+template <int N, int E>
 void set_plane(Plan& p) {
-  p.plane_step = k_plane_fast<N, E, CP, false>;
-  p.plane_emit = k_plane_fast<N, E, CP, true>;
+  p.plane_step = k_plane_fast<N, E, false>;
+  p.plane_emit = k_plane_fast<N, E, true>;
   p.plane_block = dim3(N * N / (2 * E));
-  p.plane_smem = (size_t)2 * CP * PlaneCfg<N>::BUF * sizeof(float2);
+  p.plane_smem = (size_t)2 * PlaneCfg<N>::BUF * sizeof(float2);
   p.plane_fast = true;
 }
 
-template <int NZ, int E, int TYL>
-void set_line(Plan& p, int nx, int y2, int L, int n_geoms) {
+template <int NZ, int E, int TYL, int LT>
+void set_line_lt(Plan& p, int nx, int y2) {
   using C = PencilCfg<NZ, E, TYL>;
-  p.line_step = k_pencil<NZ, E, TYL, true, false>;
-  p.line_init = k_pencil<NZ, E, TYL, false, false>;
-  p.line_delta = k_pencil<NZ, E, TYL, false, true>;
-  p.line_grid = dim3(nx * (y2 / TYL), n_geoms);
+  p.line_step = k_pencil<NZ, E, TYL, LT, true, false>;
+  p.line_init = k_pencil<NZ, E, TYL, LT, false, false>;
+  p.line_delta = k_pencil<NZ, E, TYL, LT, false, true>;
+  p.line_grid = dim3(nx * (y2 / TYL));
   p.line_block = dim3(C::THREADS);
-  p.line_smem = (size_t)2 * C::FIELD * sizeof(float2) + (size_t)std::max(1, L) * TYL * C::T * sizeof(double2);
+  p.line_smem = (size_t)2 * C::FIELD * sizeof(float2) + (size_t)LT * TYL * C::T * sizeof(double2);
   p.line_fast = true;
   p.ty = TYL;
 }
+template <int NZ, int E, int TYL>
+void set_line(Plan& p, int nx, int y2, int L) {
+  if (L <= 2) set_line_lt<NZ, E, TYL, 2>(p, nx, y2);
+  else set_line_lt<NZ, E, TYL, kMaxLayers>(p, nx, y2);
+}
 
-Plan make_plan(int nx, int ny, int nz, int L, int n_geoms, bool force_generic) {
+Plan make_plan(int nx, int ny, int nz, int L, bool force_generic) {
   Plan p;
   const int y2 = ny / 2;
   if (!force_generic && nx == ny) {
-    if (nx == 32) set_plane<32, 8, 3>(p);
-    else if (nx == 64) set_plane<64, 8, 3>(p);
-    else if (nx == 128) set_plane<128, 16, 1>(p);
+    if (nx == 32) set_plane<32, 8>(p);
+    else if (nx == 64) set_plane<64, 8>(p);
+    else if (nx == 128) set_plane<128, 16>(p);
   }
   if (!p.plane_fast) {
     p.plane_step = k_plane<false>;
     p.plane_emit = k_plane<true>;
     p.plane_block = dim3(256);
-    p.plane_smem = (size_t)3 * (nx / 2) * (ny + 1) * sizeof(float2);
+    p.plane_smem = (size_t)2 * (nx / 2) * (ny + 1) * sizeof(float2);
   }
   if (!force_generic) {
-    if (nz == 256 && y2 % 8 == 0) set_line<256, 16, 8>(p, nx, y2, L, n_geoms);
-    else if (nz == 128 && y2 % 16 == 0) set_line<128, 16, 16>(p, nx, y2, L, n_geoms);
-    else if (nz == 64 && y2 % 16 == 0) set_line<64, 8, 16>(p, nx, y2, L, n_geoms);
-    else if (nz == 32 && y2 % 16 == 0) set_line<32, 8, 16>(p, nx, y2, L, n_geoms);
+    if (nz == 256 && y2 % 8 == 0) set_line<256, 16, 8>(p, nx, y2, L);
+    else if (nz == 128 && y2 % 16 == 0) set_line<128, 16, 16>(p, nx, y2, L);
+    else if (nz == 64 && y2 % 16 == 0) set_line<64, 8, 16>(p, nx, y2, L);
+    else if (nz == 32 && y2 % 16 == 0) set_line<32, 8, 16>(p, nx, y2, L);
   }
   if (!p.line_fast) {
     p.ty = pick_ty(y2);
     p.line_step = k_spectral<true, false>;
     p.line_init = k_spectral<false, false>;
     p.line_delta = k_spectral<false, true>;
-    p.line_grid = dim3(nx * (y2 / p.ty), n_geoms);
+    p.line_grid = dim3(nx * (y2 / p.ty));
     p.line_block = dim3(32 * p.ty);
     p.line_smem = (size_t)3 * nz * p.ty * sizeof(float2) + (size_t)std::max(1, L) * p.ty * 32 * sizeof(double2);
   }
@@ -203,7 +214,7 @@ Plan make_plan(int nx, int ny, int nz, int L, int n_geoms, bool force_generic) {
 }  // namespace
 
 // bytes wt_solve_H needs for this geometry (its region + one descriptor slot + the step counter)
-size_t wt_solve_workspace_bytes(const wt_geometry* g) { return make_layout(g).total + align_up(sizeof(GeomDev)) + 256; }
+size_t wt_solve_workspace_bytes(const wt_geometry* g) { return make_layout(g).total + 256; }
 
 extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* H_dev, size_t H_bytes_each,
                           void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
@@ -225,7 +236,7 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     regions += make_layout(g).total;
     max_sub = std::max(max_sub, g->n_sub);
   }
-  const size_t need = regions + align_up((size_t)n_geoms * sizeof(GeomDev)) + 256;
+  const size_t need = regions + 256;
   const size_t hbytes = (size_t)g0->nx * g0->ny * g0->nz * g0->nt * 12;
   if (H_bytes_each < hbytes) { wt_set_error("wt_solve_H: H_bytes_each too small"); return WT_EINVAL; }
   if (((uintptr_t)workspace_dev) % 256 != 0) { wt_set_error("wt_solve_H: workspace not 256-byte aligned"); return WT_EINVAL; }
@@ -242,12 +253,13 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     maxG = std::max(maxG, (int)groups[i].grp_x.size());
     maxGL = std::max(maxGL, groups[i].max_per_layer);
   }
-  const Plan plan = make_plan(nx, ny, nz, maxL, n_geoms, env_flag("WTIDE_GENERIC"));
-  const size_t sm_padpot = (size_t)(kPadChunks + 1) * y2 * sizeof(double2);
-  const size_t sm_inject = (size_t)std::max(1, maxGL) * y2 * sizeof(double2);
+  const Plan plan = make_plan(nx, ny, nz, maxL, env_flag("WTIDE_GENERIC"));
+  // boundary adjust: one cluster launch per substep for small pad sets, three grid-wide launches otherwise
+  const BndSmem bsm = bnd_smem(nx, ny, maxGL, maxB);
+  const bool bnd_cluster = maxB <= 640 && !env_flag("WTIDE_SPLIT_BOUNDARY");
   const size_t sm_tr = (size_t)kStageSlots * 3 * std::max(nx, ny) * sizeof(float);
   const size_t kMaxSmem = 227 * 1024;
-  if (plan.plane_smem > kMaxSmem || plan.line_smem > kMaxSmem || sm_padpot > kMaxSmem || sm_inject > kMaxSmem || sm_tr > kMaxSmem) {
+  if (plan.plane_smem > kMaxSmem || plan.line_smem > kMaxSmem || bsm.total > kMaxSmem || sm_tr > kMaxSmem) {
     wt_set_error("wt_solve_H: grid too large for the shared-memory tiles (nx*ny <= 128*128, nz <= 1024)"); return WT_EINVAL;
   }
 
@@ -268,30 +280,29 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   std::vector<double2> twxd, twyd, twzd;
   twid(nx, twx, twxd); twid(ny, twy, twyd); twid(nz, twz, twzd);
 
-  // ---- upload static tables, build the device descriptors ------------------------------------
+  // ---- upload static tables, build the descriptors (which travel as kernel parameters) -----------
   std::vector<GeomDev> hd(n_geoms);
   char* base = (char*)workspace_dev;
   size_t off = 0;
-  std::vector<std::vector<uint8_t>> sig_t(n_geoms);
-  std::vector<std::vector<float>> kf(3 * n_geoms);
+  std::vector<uint8_t> sig_t;
+  std::vector<float> kxf, kyf, kzf;
   for (int i = 0; i < n_geoms; ++i) {
     const wt_geometry* g = geoms[i];
     const Layout lo = make_layout(g);
     const PadGroups& pg = groups[i];
     char* b = base + off;
     const int B = (int)g->pad_pot.size(), L = (int)g->layers.size();
-    sig_t[i].resize(g->sig_id.size());
+    sig_t.resize(g->sig_id.size());
     for (int z = 0; z < nz; ++z)
       for (int x = 0; x < nx; ++x)
-        for (int y = 0; y < ny; ++y) sig_t[i][((size_t)z * ny + y) * nx + x] = g->sig_id[((size_t)z * nx + x) * ny + y];
-    std::vector<float>&kxf = kf[3 * i], &kyf = kf[3 * i + 1], &kzf = kf[3 * i + 2];
+        for (int y = 0; y < ny; ++y) sig_t[((size_t)z * ny + y) * nx + x] = g->sig_id[((size_t)z * nx + x) * ny + y];
     kxf.assign(g->kx.begin(), g->kx.end()); kyf.assign(g->ky.begin(), g->ky.end()); kzf.assign(g->kz.begin(), g->kz.end());
-    CK(upload(b, lo.sig_id, g->sig_id, st)); CK(upload(b, lo.sig_t, sig_t[i], st)); CK(upload(b, lo.sdt, g->sdt, st));
+    // (cudaMemcpyAsync from pageable memory has staged the source before it returns)
+    CK(upload(b, lo.sig_id, g->sig_id, st)); CK(upload(b, lo.sig_t, sig_t, st)); CK(upload(b, lo.sdt, g->sdt, st));
     CK(upload(b, lo.gt, g->gt, st)); CK(upload(b, lo.gzt, g->gzt, st));
-    CK(upload(b, lo.ainv, g->ainv, st)); CK(upload(b, lo.pad_pot, g->pad_pot, st)); CK(upload(b, lo.pad_y, pg.pad_y, st));
+    CK(upload(b, lo.ainv, pg.ainv, st)); CK(upload(b, lo.pad_pot, pg.pad_pot, st)); CK(upload(b, lo.pad_y, pg.pad_y, st));
     CK(upload(b, lo.grp_x, pg.grp_x, st)); CK(upload(b, lo.grp_layer, pg.grp_layer, st));
-    CK(upload(b, lo.grp_off, pg.grp_off, st)); CK(upload(b, lo.grp_pad, pg.grp_pad, st));
-    CK(upload(b, lo.layer_goff, pg.layer_goff, st));
+    CK(upload(b, lo.grp_off, pg.grp_off, st)); CK(upload(b, lo.layer_goff, pg.layer_goff, st));
     CK(upload(b, lo.kxd, g->kx, st)); CK(upload(b, lo.kyd, g->ky, st)); CK(upload(b, lo.kzd, g->kz, st));
     CK(upload(b, lo.kxf, kxf, st)); CK(upload(b, lo.kyf, kyf, st)); CK(upload(b, lo.kzf, kzf, st));
     CK(upload(b, lo.twx, twx, st)); CK(upload(b, lo.twy, twy, st)); CK(upload(b, lo.twz, twz, st));
@@ -301,14 +312,15 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     d.gt = (const float*)(b + lo.gt); d.gzt = (const float*)(b + lo.gzt);
     d.ainv = (const double*)(b + lo.ainv); d.pad_pot = (const double*)(b + lo.pad_pot); d.pad_y = (const int*)(b + lo.pad_y);
     d.grp_x = (const int*)(b + lo.grp_x); d.grp_layer = (const int*)(b + lo.grp_layer);
-    d.grp_off = (const int*)(b + lo.grp_off); d.grp_pad = (const int*)(b + lo.grp_pad);
-    d.layer_goff = (const int*)(b + lo.layer_goff);
+    d.grp_off = (const int*)(b + lo.grp_off); d.layer_goff = (const int*)(b + lo.layer_goff);
     d.kxd = (const double*)(b + lo.kxd); d.kyd = (const double*)(b + lo.kyd); d.kzd = (const double*)(b + lo.kzd);
     d.kxf = (const float*)(b + lo.kxf); d.kyf = (const float*)(b + lo.kyf); d.kzf = (const float*)(b + lo.kzf);
     d.twx = (const float2*)(b + lo.twx); d.twy = (const float2*)(b + lo.twy); d.twz = (const float2*)(b + lo.twz);
     d.twxd = (const double2*)(b + lo.twxd); d.twyd = (const double2*)(b + lo.twyd); d.twzd = (const double2*)(b + lo.twzd);
     d.rhat = (double2*)(b + lo.rhat); d.rhat_prev = (double2*)(b + lo.rhat_prev);
-    d.m0 = (float2*)(b + lo.m0); d.m1 = (float2*)(b + lo.m1); d.e0 = (float2*)(b + lo.e0); d.e1 = (float2*)(b + lo.e1);
+    d.v0 = (float2*)(b + lo.v0); d.v1 = (float2*)(b + lo.v1);
+    d.m0 = (float2*)(b + lo.m0); d.m1 = (float2*)(b + lo.m1); d.m2 = (float2*)(b + lo.m2);
+    d.e0 = (float2*)(b + lo.e0); d.e1 = (float2*)(b + lo.e1);
     d.pl = (double2*)(b + lo.pl); d.pl_e = (double2*)(b + lo.pl_e);
     d.rhs = (double*)(b + lo.rhs); d.q = (double*)(b + lo.q); d.qh = (float2*)(b + lo.qh);
     d.stage = (float*)(b + lo.stage);
@@ -317,12 +329,17 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     d.B = B; d.L = L; d.G = (int)pg.grp_x.size(); d.n_sub = g->n_sub; d.inv_dt = (float)(1.0 / g->dt);
     off += lo.total;
   }
-  GeomDev* dgeoms = (GeomDev*)(base + off);
-  CK(cudaMemcpyAsync(dgeoms, hd.data(), (size_t)n_geoms * sizeof(GeomDev), cudaMemcpyHostToDevice, st));
-  int* dstep = (int*)(base + off + align_up((size_t)n_geoms * sizeof(GeomDev)));
+  int* dstep = (int*)(base + off);
   gd.step = dstep;
   CK(cudaMemsetAsync(dstep, 0, sizeof(int), st));
-  // the uploads above read pageable host vectors: cudaMemcpyAsync has staged them before it returns
+  // descriptors in launch batches of kBatch geometries
+  const int n_batches = (n_geoms + kBatch - 1) / kBatch;
+  std::vector<GeomBatch> batches(n_batches);
+  std::vector<int> batch_n(n_batches);
+  for (int bi = 0; bi < n_batches; ++bi) {
+    batch_n[bi] = std::min(kBatch, n_geoms - bi * kBatch);
+    for (int k = 0; k < kBatch; ++k) batches[bi].g[k] = hd[bi * kBatch + std::min(k, batch_n[bi] - 1)];
+  }
 
   // ---- launch configuration -------------------------------------------------------------------
   auto set_smem = [&](const void* fn, size_t bytes) -> cudaError_t {
@@ -331,41 +348,71 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   CK(set_smem((const void*)plan.plane_step, plan.plane_smem)); CK(set_smem((const void*)plan.plane_emit, plan.plane_smem));
   CK(set_smem((const void*)plan.line_step, plan.line_smem)); CK(set_smem((const void*)plan.line_init, plan.line_smem));
   CK(set_smem((const void*)plan.line_delta, plan.line_smem));
-  CK(set_smem((const void*)k_padpot, sm_padpot)); CK(set_smem((const void*)k_inject, sm_inject));
+  CK(set_smem((const void*)k_boundary<0>, bsm.total)); CK(set_smem((const void*)k_boundary<1>, bsm.total));
+  CK(set_smem((const void*)k_boundary<2>, bsm.total)); CK(set_smem((const void*)k_boundary<3>, bsm.total));
   CK(set_smem((const void*)k_transpose<false>, sm_tr)); CK(set_smem((const void*)k_transpose<true>, sm_tr));
-  const dim3 g_plane(nz, n_geoms);
-  const dim3 g_pot(std::max(1, maxG), n_geoms);
-  const dim3 g_mv((maxB * 32 + 255) / 256, n_geoms);
-  const dim3 g_inj((nx + kInjKx - 1) / kInjKx, std::max(1, maxL), n_geoms);
-  const dim3 g_tr(plan.plane_fast ? nz * ny : nz * nx, n_geoms);
+  const int n_tr = plan.plane_fast ? nz * ny : nz * nx;
   const size_t half = (size_t)nx * nz * y2;
+  const int bnd_units3 = std::max(1, maxL) * ((nx + kBndKx - 1) / kBndKx);
+  const int bnd_rows = (maxB + kBndThreads / 32 - 1) / (kBndThreads / 32);
 
   long long launches = 0;
+  cudaError_t launch_err = cudaSuccess;
+  auto note = [&](cudaError_t e) { if (e != cudaSuccess && launch_err == cudaSuccess) launch_err = e; };
   auto boundary = [&](int s, int emit, double flag) {
     if (maxB == 0) return;
-    launches += 3;
-    k_padpot<<<g_pot, 256, sm_padpot, st>>>(gd, dgeoms, s, emit, flag);
-    k_matvec<<<g_mv, 256, 0, st>>>(dgeoms, s);
-    k_inject<<<g_inj, 256, sm_inject, st>>>(gd, dgeoms, s);
+    for (int bi = 0; bi < n_batches; ++bi) {
+      const GeomBatch& gb = batches[bi];
+      const int nb = batch_n[bi];
+      if (bnd_cluster) {
+        ++launches;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(kBndCluster, nb); cfg.blockDim = dim3(kBndThreads); cfg.dynamicSmemBytes = bsm.total; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = kBndCluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        note(cudaLaunchKernelEx(&cfg, k_boundary<0>, gb, gd, maxGL, s, emit, flag));
+      } else {
+        launches += 3;
+        k_boundary<1><<<dim3(std::max(1, maxG), nb), kBndThreads, bsm.total, st>>>(gb, gd, maxGL, s, emit, flag);
+        k_boundary<2><<<dim3(std::max(1, bnd_rows), nb), kBndThreads, bsm.total, st>>>(gb, gd, maxGL, s, emit, flag);
+        k_boundary<3><<<dim3(bnd_units3, nb), kBndThreads, bsm.total, st>>>(gb, gd, maxGL, s, emit, flag);
+      }
+    }
+  };
+  auto plane = [&](PlaneFn fn, int s) {
+    for (int bi = 0; bi < n_batches; ++bi) {
+      ++launches;
+      const dim3 grid = plan.plane_fast ? dim3(nz, 3, batch_n[bi]) : dim3(nz, batch_n[bi]);
+      fn<<<grid, plan.plane_block, plan.plane_smem, st>>>(batches[bi], gd, s);
+    }
+  };
+  auto line = [&](LineFn fn, int s, int emit) {
+    for (int bi = 0; bi < n_batches; ++bi) {
+      ++launches;
+      fn<<<dim3(plan.line_grid.x, batch_n[bi]), plan.line_block, plan.line_smem, st>>>(batches[bi], gd, s, emit);
+    }
   };
   auto emit_step = [&](bool first) {
     // H[n] from the increment of the charge since the previous output step (the prompt response
     // H[0] from the pads alone: r = 0, pads at v_w); n is read from the device counter
-    launches += 4;
-    const LineFn line_emit = first ? plan.line_init : plan.line_delta;
-    line_emit<<<plan.line_grid, plan.line_block, plan.line_smem, st>>>(gd, dgeoms, 0, 1);
+    line(first ? plan.line_init : plan.line_delta, 0, 1);
     boundary(0, 1, first ? 1.0 : 0.0);
-    plan.plane_emit<<<g_plane, plan.plane_block, plan.plane_smem, st>>>(gd, dgeoms, 0);
-    if (plan.plane_fast) k_transpose<true><<<g_tr, 256, sm_tr, st>>>(gd, dgeoms);
-    else                 k_transpose<false><<<g_tr, 256, sm_tr, st>>>(gd, dgeoms);
+    plane(plan.plane_emit, 0);
+    for (int bi = 0; bi < n_batches; ++bi) {
+      ++launches;
+      if (plan.plane_fast) k_transpose<true><<<dim3(n_tr, batch_n[bi]), 256, sm_tr, st>>>(batches[bi], gd);
+      else                 k_transpose<false><<<dim3(n_tr, batch_n[bi]), 256, sm_tr, st>>>(batches[bi], gd);
+    }
+    ++launches;
     k_advance<<<1, 1, 0, st>>>(dstep);
   };
   auto output_step = [&]() {
     for (int s = 0; s < max_sub; ++s) {
       boundary(s, 0, 1.0);
-      launches += 2;
-      plan.plane_step<<<g_plane, plan.plane_block, plan.plane_smem, st>>>(gd, dgeoms, s);
-      plan.line_step<<<plan.line_grid, plan.line_block, plan.line_smem, st>>>(gd, dgeoms, s, 0);
+      plane(plan.plane_step, s);
+      line(plan.line_step, s, 0);
     }
     emit_step(false);
   };
@@ -376,9 +423,9 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     if (hd[i].L > 0) CK(cudaMemsetAsync(hd[i].qh, 0, (size_t)hd[i].L * nx * y2 * sizeof(float2), st));
   }
   emit_step(true);
-  ++launches;
-  plan.line_init<<<plan.line_grid, plan.line_block, plan.line_smem, st>>>(gd, dgeoms, 0, 0);
+  line(plan.line_init, 0, 0);
   CK(cudaGetLastError());
+  CK(launch_err);
 
   const int n_out = nt - 1;
   if (n_out >= 2 && !env_flag("WTIDE_NO_GRAPH")) {
@@ -389,7 +436,9 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     CK(cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
     output_step();
     cudaError_t ec = cudaStreamEndCapture(st, &graph);
+    if (ec == cudaSuccess) ec = launch_err;
     if (ec != cudaSuccess || !graph) {
+      if (graph) cudaGraphDestroy(graph);
       wt_set_error(std::string("wt_solve_H: stream capture failed: ") + cudaGetErrorString(ec)); return WT_ECUDA;
     }
     const long long per_step = launches - before;
@@ -408,6 +457,7 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     for (int n = 0; n < n_out; ++n) output_step();
   }
   CK(cudaGetLastError());
+  CK(launch_err);
   g_wt_launches += launches;
   wt_set_error("");
   return WT_OK;

@@ -14,8 +14,8 @@ namespace wt {
 //   V~_rho at the pad layers in fp64 (a3);  inverse z DFT of V^ and -i kz V^  (a5, z part)
 // ------------------------------------------------------------------------------------------------
 template <bool APPLY_J, bool DELTA>
-__global__ void __launch_bounds__(256) k_spectral(GridDev gd, const GeomDev* __restrict__ geoms, int substep, int emit) {
-  const GeomDev& g = geoms[blockIdx.y];
+__global__ void __launch_bounds__(256) k_spectral(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emit) {
+  const GeomDev& g = gb.g[blockIdx.y];
   if (substep >= g.n_sub) return;
   const int nx = gd.nx, nz = gd.nz, y2 = gd.y2, TY = gd.ty;
   const int tiles = y2 / TY;
@@ -28,8 +28,8 @@ __global__ void __launch_bounds__(256) k_spectral(GridDev gd, const GeomDev* __r
   float2* b1 = b0 + nelem;
   float2* b2 = b1 + nelem;
   double2* red = reinterpret_cast<double2*>(b2 + nelem);   // [L][TY][32]
-  float2* mV = emit ? g.e0 : g.m0;
-  float2* mE = emit ? g.e1 : g.m1;
+  float2* mV = emit ? g.e0 : g.v0;
+  float2* mE = emit ? g.e1 : g.v1;
   const size_t slab = (size_t)kx * nz * y2 + ky0;
 
   float2 *dres, *jres, *vb;
@@ -37,8 +37,9 @@ __global__ void __launch_bounds__(256) k_spectral(GridDev gd, const GeomDev* __r
     for (int t = tid; t < nelem; t += bd) {
       const int z = t / TY, ty = t - z * TY;
       const size_t gi = slab + (size_t)z * y2 + ty;
-      b0[t] = g.m0[gi];
-      b2[t] = g.m1[gi];
+      const float2 dx = g.m0[gi], dy = g.m1[gi];
+      b0[t] = make_float2(dx.x + dy.x, dx.y + dy.y);   // D~ = i kx J~x + i ky J~y
+      b2[t] = g.m2[gi];
     }
     __syncthreads();
     dres = fft_lines<float2>(b0, b1, nz, TY, 1, TY, g.twz, false);
@@ -117,15 +118,15 @@ __global__ void __launch_bounds__(256) k_spectral(GridDev gd, const GeomDev* __r
 
 // ------------------------------------------------------------------------------------------------
 // k_plane: xy-plane transforms.  grid (nz, n_geoms), block 256.
-// Shared memory: three buffers of (nx/2)*(ny+1) float2 used either as a half-spectrum plane
+// Shared memory: two buffers of (nx/2)*(ny+1) float2 used either as a half-spectrum plane
 // [kx][ky] (row stride y2) or as nx/2 complex lines of length ny, each packing the two real
 // x-rows 2p (real part) and 2p+1 (imaginary part), line stride ny+1 (odd: conflict free).
 //   V~ = V~_rho + sum_l Q^_l g~(z - z_l)  (a4);  E~ = -i kappa V~;  inverse xy DFT  (a5);
-//   J = s dt_int E  (a6);  forward xy DFT;  D~ = i kx J~x + i ky J~y.   EMIT: H[n] = E/dt  (a8)
+//   J = s dt_int E  (a6);  forward xy DFT;  out: i kx J~x, i ky J~y, J~z.   EMIT: H[n] = E/dt  (a8)
 // ------------------------------------------------------------------------------------------------
 template <bool EMIT>
-__global__ void __launch_bounds__(256) k_plane(GridDev gd, const GeomDev* __restrict__ geoms, int substep) {
-  const GeomDev& g = geoms[blockIdx.y];
+__global__ void __launch_bounds__(256) k_plane(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
+  const GeomDev& g = gb.g[blockIdx.y];
   if (substep >= g.n_sub) return;
   const int nx = gd.nx, ny = gd.ny, nz = gd.nz, y2 = gd.y2;
   const int z = blockIdx.x;
@@ -134,11 +135,10 @@ __global__ void __launch_bounds__(256) k_plane(GridDev gd, const GeomDev* __rest
   const int nspec = nx * y2, nline = hx * ny;
   const int bufsz = hx * nyp;
   extern __shared__ __align__(16) unsigned char smraw[];
-  float2* dacc = reinterpret_cast<float2*>(smraw);
-  float2* w1 = dacc + bufsz;
+  float2* w1 = reinterpret_cast<float2*>(smraw);
   float2* w2 = w1 + bufsz;
-  const float2* mV = EMIT ? g.e0 : g.m0;
-  const float2* mE = EMIT ? g.e1 : g.m1;
+  const float2* mV = EMIT ? g.e0 : g.v0;
+  const float2* mE = EMIT ? g.e1 : g.v1;
   const int L = g.L;
   const int slot = EMIT ? (*gd.step % kStageSlots) : 0;
 
@@ -219,18 +219,15 @@ __global__ void __launch_bounds__(256) k_plane(GridDev gd, const GeomDev* __rest
     for (int t = tid; t < nspec; t += bd) {
       const int kx = t / y2, ky = t - kx * y2;
       const float2 j = jt[t];
+      const size_t gi = ((size_t)kx * nz + z) * y2 + ky;
       if (comp == 0) {
         const float kap = g.kxf[kx];
-        dacc[t] = make_float2(-kap * j.y, kap * j.x);
+        g.m0[gi] = make_float2(-kap * j.y, kap * j.x);     // i kx J~x
       } else if (comp == 1) {
         const float kap = g.kyf[ky];
-        float2 d = dacc[t];
-        d.x -= kap * j.y; d.y += kap * j.x;
-        dacc[t] = d;
+        g.m1[gi] = make_float2(-kap * j.y, kap * j.x);     // i ky J~y
       } else {
-        const size_t gi = ((size_t)kx * nz + z) * y2 + ky;
-        g.m1[gi] = j;
-        g.m0[gi] = dacc[t];
+        g.m2[gi] = j;
       }
     }
     __syncthreads();
@@ -244,11 +241,11 @@ __global__ void __launch_bounds__(256) k_plane(GridDev gd, const GeomDev* __rest
 // grid (nz*ny, n_geoms).  block 256; dynamic smem kStageSlots*3*max(nx,ny) floats.
 // ------------------------------------------------------------------------------------------------
 template <bool YX>
-__global__ void __launch_bounds__(256) k_transpose(GridDev gd, const GeomDev* __restrict__ geoms) {
+__global__ void __launch_bounds__(256) k_transpose(const __grid_constant__ GeomBatch gb, GridDev gd) {
   const int n = *gd.step;
   if (!((n + 1) % kStageSlots == 0 || n == gd.nt - 1)) return;
   const int cnt = n % kStageSlots + 1, t0 = n - cnt + 1;
-  const GeomDev& g = geoms[blockIdx.y];
+  const GeomDev& g = gb.g[blockIdx.y];
   const int nx = gd.nx, ny = gd.ny, nz = gd.nz, nt = gd.nt;
   const int na = YX ? ny : nx;        // outer in-plane index (one per CTA)
   const int nb = YX ? nx : ny;        // inner in-plane index (contiguous in the staging)
