@@ -79,11 +79,12 @@ PadGroups make_groups(const wt_geometry* g) {
     o.max_per_layer = std::max(o.max_per_layer, o.layer_goff[l + 1]);
     o.layer_goff[l + 1] += o.layer_goff[l];
   }
-  o.pad_y.resize(B); o.pad_pot.resize(B); o.ainv.resize((size_t)B * B);
+  const int Bs = (B + 1) & ~1;    // even row stride: rows and row slices start 16-byte aligned
+  o.pad_y.resize(B); o.pad_pot.resize(B); o.ainv.assign((size_t)B * Bs, 0.0);
   for (int i = 0; i < B; ++i) {
     o.pad_y[i] = g->pad_nodes[3 * o.perm[i] + 1];
     o.pad_pot[i] = g->pad_pot[o.perm[i]];
-    for (int k = 0; k < B; ++k) o.ainv[(size_t)i * B + k] = g->ainv[(size_t)o.perm[i] * B + o.perm[k]];
+    for (int k = 0; k < B; ++k) o.ainv[(size_t)i * Bs + k] = g->ainv[(size_t)o.perm[i] * B + o.perm[k]];
   }
   return o;
 }
@@ -104,7 +105,7 @@ Layout make_layout(const wt_geometry* g) {
   size_t p = 0;
   auto take = [&](size_t bytes) { size_t at = p; p = align_up(p + bytes); return at; };
   o.sig_id = take(N); o.sig_t = take(N); o.sdt = take(256 * 4); o.gt = take(half * 4); o.gzt = take(half * 4);
-  o.ainv = take(B * B * 8); o.pad_pot = take(B * 8); o.pad_y = take(B * 4);
+  o.ainv = take(B * ((B + 1) & ~(size_t)1) * 8); o.pad_pot = take(B * 8); o.pad_y = take(B * 4);
   o.grp_x = take(B * 4); o.grp_layer = take(B * 4); o.grp_off = take((B + 1) * 4);
   o.layer_goff = take((L + 1) * 4);
   o.kxd = take(nx * 8); o.kyd = take(y2 * 8); o.kzd = take(nz * 8);
@@ -214,7 +215,7 @@ Plan make_plan(int nx, int ny, int nz, int L, bool force_generic) {
 }  // namespace
 
 // bytes wt_solve_H needs for this geometry (its region + one descriptor slot + the step counter)
-size_t wt_solve_workspace_bytes(const wt_geometry* g) { return make_layout(g).total + 256; }
+size_t wt_solve_workspace_bytes(const wt_geometry* g) { return make_layout(g).total + 4096; }
 
 extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* H_dev, size_t H_bytes_each,
                           void* workspace_dev, size_t workspace_bytes, void* cuda_stream) {
@@ -236,7 +237,7 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     regions += make_layout(g).total;
     max_sub = std::max(max_sub, g->n_sub);
   }
-  const size_t need = regions + 256;
+  const size_t need = regions + 4096;
   const size_t hbytes = (size_t)g0->nx * g0->ny * g0->nz * g0->nt * 12;
   if (H_bytes_each < hbytes) { wt_set_error("wt_solve_H: H_bytes_each too small"); return WT_EINVAL; }
   if (((uintptr_t)workspace_dev) % 256 != 0) { wt_set_error("wt_solve_H: workspace not 256-byte aligned"); return WT_EINVAL; }
@@ -254,11 +255,42 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     maxGL = std::max(maxGL, groups[i].max_per_layer);
   }
   const Plan plan = make_plan(nx, ny, nz, maxL, env_flag("WTIDE_GENERIC"));
-  // boundary adjust: one cluster launch per substep for small pad sets, three grid-wide launches otherwise
   const BndSmem bsm = bnd_smem(nx, ny, maxGL, maxB);
-  const bool bnd_cluster = maxB <= 640 && !env_flag("WTIDE_SPLIT_BOUNDARY");
-  const size_t sm_tr = (size_t)kStageSlots * 3 * std::max(nx, ny) * sizeof(float);
   const size_t kMaxSmem = 227 * 1024;
+  const size_t sm_tr = (size_t)kStageSlots * 3 * std::max(nx, ny) * sizeof(float);
+  // boundary adjust: one cluster launch per substep for small pad sets (16 CTAs where the device can
+  // co-schedule the non-portable size, else 8), three grid-wide launches otherwise
+  const bool pow2 = (nx & (nx - 1)) == 0 && (ny & (ny - 1)) == 0;
+  const void* bnd_fn = pow2 ? (const void*)k_boundary_cluster<true> : (const void*)k_boundary_cluster<false>;
+  const int maxBs = (maxB + 1) & ~1;
+  int bnd_cl = 8;
+  BndClSmem bcl;
+  int ainv_in_smem = 1;
+  auto size_cluster = [&](int cl) {
+    bnd_cl = cl; ainv_in_smem = 1;
+    bcl = bnd_cl_smem(nx, ny, kMaxLayers, maxG, maxB, maxBs, cl, true);
+    if (bcl.total > 200 * 1024) { bcl = bnd_cl_smem(nx, ny, kMaxLayers, maxG, maxB, maxBs, cl, false); ainv_in_smem = 0; }
+  };
+  size_cluster(16);
+  bool bnd_cluster = maxB > 0 && maxB <= 640 && !env_flag("WTIDE_SPLIT_BOUNDARY");
+  if (bnd_cluster) {
+    bool ok16 = !env_flag("WTIDE_CLUSTER8") && bcl.total <= kMaxSmem &&
+                cudaFuncSetAttribute(bnd_fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess &&
+                cudaFuncSetAttribute(bnd_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bcl.total) == cudaSuccess;
+    if (ok16) {
+      cudaLaunchConfig_t q = {};
+      q.gridDim = dim3(16, 1); q.blockDim = dim3(kBclThreads); q.dynamicSmemBytes = bcl.total;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeClusterDimension;
+      at[0].val.clusterDim.x = 16; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+      q.attrs = at; q.numAttrs = 1;
+      int n_clusters = 0;
+      ok16 = cudaOccupancyMaxActiveClusters(&n_clusters, bnd_fn, &q) == cudaSuccess && n_clusters >= 1;
+    }
+    cudaGetLastError();
+    if (!ok16) size_cluster(8);
+    if (bcl.total > kMaxSmem) bnd_cluster = false;
+  }
   if (plan.plane_smem > kMaxSmem || plan.line_smem > kMaxSmem || bsm.total > kMaxSmem || sm_tr > kMaxSmem) {
     wt_set_error("wt_solve_H: grid too large for the shared-memory tiles (nx*ny <= 128*128, nz <= 1024)"); return WT_EINVAL;
   }
@@ -326,11 +358,13 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     d.stage = (float*)(b + lo.stage);
     d.H = H_dev[i];
     for (int l = 0; l < kMaxLayers; ++l) d.layers[l] = (l < L) ? g->layers[l] : 0;
-    d.B = B; d.L = L; d.G = (int)pg.grp_x.size(); d.n_sub = g->n_sub; d.inv_dt = (float)(1.0 / g->dt);
+    for (int l = 0; l <= kMaxLayers; ++l) d.lgoff[l] = pg.layer_goff[std::min(l, L)];
+    d.B = B; d.Bs = (B + 1) & ~1; d.L = L; d.G = (int)pg.grp_x.size(); d.n_sub = g->n_sub; d.inv_dt = (float)(1.0 / g->dt);
     off += lo.total;
   }
   int* dstep = (int*)(base + off);
   gd.step = dstep;
+  gd.stamps = env_flag("WTIDE_STAMPS") ? (long long*)(base + off + 256) : nullptr;
   CK(cudaMemsetAsync(dstep, 0, sizeof(int), st));
   // descriptors in launch batches of kBatch geometries
   const int n_batches = (n_geoms + kBatch - 1) / kBatch;
@@ -348,7 +382,8 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   CK(set_smem((const void*)plan.plane_step, plan.plane_smem)); CK(set_smem((const void*)plan.plane_emit, plan.plane_smem));
   CK(set_smem((const void*)plan.line_step, plan.line_smem)); CK(set_smem((const void*)plan.line_init, plan.line_smem));
   CK(set_smem((const void*)plan.line_delta, plan.line_smem));
-  CK(set_smem((const void*)k_boundary<0>, bsm.total)); CK(set_smem((const void*)k_boundary<1>, bsm.total));
+  if (bnd_cluster) CK(set_smem(bnd_fn, bcl.total));
+  CK(set_smem((const void*)k_boundary<1>, bsm.total));
   CK(set_smem((const void*)k_boundary<2>, bsm.total)); CK(set_smem((const void*)k_boundary<3>, bsm.total));
   CK(set_smem((const void*)k_transpose<false>, sm_tr)); CK(set_smem((const void*)k_transpose<true>, sm_tr));
   const int n_tr = plan.plane_fast ? nz * ny : nz * nx;
@@ -356,6 +391,7 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   const int bnd_units3 = std::max(1, maxL) * ((nx + kBndKx - 1) / kBndKx);
   const int bnd_rows = (maxB + kBndThreads / 32 - 1) / (kBndThreads / 32);
 
+  const int dbg_skip = std::getenv("WTIDE_DBG_SKIP") ? std::atoi(std::getenv("WTIDE_DBG_SKIP")) : 0;
   long long launches = 0;
   cudaError_t launch_err = cudaSuccess;
   auto note = [&](cudaError_t e) { if (e != cudaSuccess && launch_err == cudaSuccess) launch_err = e; };
@@ -367,12 +403,13 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
       if (bnd_cluster) {
         ++launches;
         cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(kBndCluster, nb); cfg.blockDim = dim3(kBndThreads); cfg.dynamicSmemBytes = bsm.total; cfg.stream = st;
+        cfg.gridDim = dim3(bnd_cl, nb); cfg.blockDim = dim3(kBclThreads); cfg.dynamicSmemBytes = bcl.total; cfg.stream = st;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = kBndCluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        at[0].val.clusterDim.x = bnd_cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
-        note(cudaLaunchKernelEx(&cfg, k_boundary<0>, gb, gd, maxGL, s, emit, flag));
+        if (pow2) note(cudaLaunchKernelEx(&cfg, k_boundary_cluster<true>, gb, gd, maxG, maxB, maxBs, ainv_in_smem, s, emit, flag));
+        else note(cudaLaunchKernelEx(&cfg, k_boundary_cluster<false>, gb, gd, maxG, maxB, maxBs, ainv_in_smem, s, emit, flag));
       } else {
         launches += 3;
         k_boundary<1><<<dim3(std::max(1, maxG), nb), kBndThreads, bsm.total, st>>>(gb, gd, maxGL, s, emit, flag);
@@ -410,9 +447,9 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   };
   auto output_step = [&]() {
     for (int s = 0; s < max_sub; ++s) {
-      boundary(s, 0, 1.0);
-      plane(plan.plane_step, s);
-      line(plan.line_step, s, 0);
+      if (!(dbg_skip & 1)) boundary(s, 0, 1.0);
+      if (!(dbg_skip & 2)) plane(plan.plane_step, s);
+      if (!(dbg_skip & 4)) line(plan.line_step, s, 0);
     }
     emit_step(false);
   };

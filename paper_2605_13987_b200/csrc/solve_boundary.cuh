@@ -9,12 +9,13 @@
 //            per group, then along x); the plane kernel multiplies it with the translated fundamental
 //            solution g~(kx, z - z_l, ky)  (the paper's V_ext in O(N) instead of O(|B| N))
 //
-// k_boundary<0> runs the three phases in ONE launch on a thread-block cluster of kBndCluster CTAs per
-// geometry (cluster barriers between the phases; small pad sets: the chain is latency bound);
+// k_boundary_cluster runs the three phases in ONE launch on a thread-block cluster of kBndCluster CTAs
+// per geometry (small pad sets: the chain is latency bound);
 // k_boundary<1|2|3> run one phase each on as many CTAs as there are work units (large pad sets:
 // Ainv is streamed by the whole chip).  Work units are strided over the CTAs of the launch.
 #pragma once
 #include <cooperative_groups.h>
+#include <cuda_pipeline.h>
 
 #include "solve_common.cuh"
 
@@ -43,7 +44,7 @@ __host__ __device__ inline BndSmem bnd_smem(int nx, int ny, int max_groups_per_l
   return s;
 }
 
-// grid (n_cta, n_geoms_in_batch), block kBndThreads.  PHASE 0: n_cta = kBndCluster = one cluster.
+// grid (n_cta, n_geoms_in_batch), block kBndThreads.
 template <int PHASE>
 __global__ void __launch_bounds__(kBndThreads)
 k_boundary(const __grid_constant__ GeomBatch gb, GridDev gd, int max_gl, int substep, int emit, double flag) {
@@ -72,7 +73,7 @@ k_boundary(const __grid_constant__ GeomBatch gb, GridDev gd, int max_gl, int sub
   }
 
   // ---- phase 1: pad potentials of the free charge ------------------------------------------------
-  if (PHASE == 0 || PHASE == 1) {
+  if (PHASE == 1) {
     double2* part = work;                               // [kBndChunks][y2]
     double2* tl = work + kBndChunks * y2;               // [y2]
     const int per = (nx + kBndChunks - 1) / kBndChunks;
@@ -116,12 +117,10 @@ k_boundary(const __grid_constant__ GeomBatch gb, GridDev gd, int max_gl, int sub
       __syncthreads();                                  // part / tl are reused by the next group
     }
   }
-  if (PHASE == 0) cooperative_groups::this_cluster().sync();
-
   // ---- phase 2: Q' = Ainv rhs ----------------------------------------------------------------------
-  if (PHASE == 0 || PHASE == 2) {
+  if (PHASE == 2) {
     for (int row = cta * kWarps + warp; row < B; row += n_cta * kWarps) {
-      const double* __restrict__ a = g.ainv + (size_t)row * B;
+      const double* __restrict__ a = g.ainv + (size_t)row * g.Bs;
       double s = 0.0;
       for (int jj = lane; jj < B; jj += 32) s += a[jj] * __ldcg(g.rhs + jj);
 #pragma unroll
@@ -129,10 +128,8 @@ k_boundary(const __grid_constant__ GeomBatch gb, GridDev gd, int max_gl, int sub
       if (lane == 0) g.q[row] = s;
     }
   }
-  if (PHASE == 0) cooperative_groups::this_cluster().sync();
-
   // ---- phase 3: spectrum of the boundary charges per pad layer -------------------------------------
-  if (PHASE == 0 || PHASE == 3) {
+  if (PHASE == 3) {
     for (int i = tid; i < B; i += kBndThreads) qs[i] = __ldcg(g.q + i);
     __syncthreads();
     const int kchunks = (nx + kBndKx - 1) / kBndKx;
@@ -170,6 +167,283 @@ k_boundary(const __grid_constant__ GeomBatch gb, GridDev gd, int max_gl, int sub
       }
     }
   }
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// k_boundary_cluster: the three phases in ONE launch on a cluster of CL CTAs per geometry (CL = 16
+// where the device grants the non-portable size, else 8), written for latency -- the chain
+// z-line kernel -> boundary -> plane kernel is serial and the pad sets are small, so what counts is
+// the number of dependent steps, not throughput:
+//   - the CTA's row slice of Ainv arrives by ONE bulk (TMA) copy, issued first and awaited before
+//     phase 2; every small table is staged in shared memory once; the first loads of pl are issued
+//     before the first barrier (their addresses come from the parameter space alone);
+//   - phase 1: each CTA owns a contiguous range of groups; rhs values are pushed into EVERY CTA's
+//     shared memory (DSMEM), so that phase 2 needs no global round trip;
+//   - phase 2: each CTA owns a contiguous range of rows of Ainv (one warp per row); Q' is pushed
+//     the same way;
+//   - phase 3: each CTA owns a contiguous range of (layer, kx) rows of Q^_l.
+// Two cluster barriers in total.  Summation orders are fixed (run-to-run deterministic).
+// POW2: nx and ny are powers of two (index arithmetic by masks instead of integer division).
+// ------------------------------------------------------------------------------------------------
+constexpr int kBclThreads = 1024;
+
+struct BndClSmem {
+  size_t bar, twx, twy, vpad, rhs, q, work, wtab, ys, gx, gl, goff, ainv, total;
+  int kc, gpc, rows, rpc;
+};
+__host__ __device__ inline BndClSmem bnd_cl_smem(int nx, int ny, int L, int G, int B, int Bs, int CL, bool ainv_in_smem) {
+  BndClSmem s;
+  const int y2 = ny / 2;
+  const int Gp = G > 0 ? G : 1, Bp = B > 0 ? B : 1, Lp = L > 0 ? L : 1;
+  s.kc = kBclThreads / y2 < 1 ? 1 : (kBclThreads / y2 > nx ? nx : kBclThreads / y2);
+  s.gpc = (Gp + CL - 1) / CL;
+  s.rows = (Bp + CL - 1) / CL;
+  s.rpc = (Lp * nx + CL - 1) / CL;
+  size_t p = 0;
+  s.bar = p; p += 16;
+  s.twx = p; p += (size_t)nx * 16;
+  s.twy = p; p += (size_t)ny * 16;
+  const size_t w1 = (size_t)(s.kc + 1) * s.gpc * y2 * 16, w3 = (size_t)Gp * y2 * 16;
+  s.work = p; p += (w1 > w3 ? w1 : w3);
+  s.wtab = p; p += (size_t)s.rpc * Gp * 16;
+  s.ainv = p; p += ainv_in_smem ? (size_t)s.rows * Bs * 8 : 0;
+  s.vpad = p; p += (size_t)Bp * 8;
+  s.rhs = p; p += (size_t)Bp * 8;
+  s.q = p; p += (size_t)Bp * 8;
+  s.ys = p; p += (size_t)Bp * 4;
+  s.gx = p; p += (size_t)Gp * 4;
+  s.gl = p; p += (size_t)Gp * 4;
+  s.goff = p; p += (size_t)(Gp + 1) * 4;
+  s.total = (p + 15) / 16 * 16;
+  return s;
+}
+
+template <bool POW2>
+__global__ void __launch_bounds__(kBclThreads, 1)
+k_boundary_cluster(const __grid_constant__ GeomBatch gb, GridDev gd, int max_g, int max_b, int max_bs, int ainv_in_smem,
+                   int substep, int emit, double flag) {
+  namespace cg = cooperative_groups;
+  const GeomDev& g = gb.g[blockIdx.y];
+  if (substep >= g.n_sub || g.B == 0) return;       // uniform over the cluster
+  cg::cluster_group cluster = cg::this_cluster();
+  cluster.barrier_arrive();                         // (waited for before the first remote store)
+#define WT_STAMP(k) do { if (gd.stamps && threadIdx.x == 0 && blockIdx.y == 0) gd.stamps[blockIdx.x * 16 + (k)] = clock64(); } while (0)
+  WT_STAMP(0);
+  const int CL = gridDim.x;                         // grid.x == cluster size
+  const int rank = blockIdx.x;
+  const int nx = gd.nx, ny = gd.ny, y2 = gd.y2, tid = threadIdx.x;
+  const int B = g.B, Bs = g.Bs, G = g.G, L = g.L;
+  auto modx = [&](int v) { return POW2 ? (v & (nx - 1)) : (v % nx); };
+  auto mody = [&](int v) { return POW2 ? (v & (ny - 1)) : (v % ny); };
+  extern __shared__ __align__(16) unsigned char smraw[];
+  const BndClSmem so = bnd_cl_smem(nx, ny, kMaxLayers, max_g, max_b, max_bs, CL, ainv_in_smem != 0);
+  double2* twx = reinterpret_cast<double2*>(smraw + so.twx);    // e^{-2 pi i k/nx}
+  double2* twy = reinterpret_cast<double2*>(smraw + so.twy);
+  double2* work = reinterpret_cast<double2*>(smraw + so.work);
+  double2* wtab = reinterpret_cast<double2*>(smraw + so.wtab);
+  double* vpad = reinterpret_cast<double*>(smraw + so.vpad);
+  double* rhs = reinterpret_cast<double*>(smraw + so.rhs);
+  double* qs = reinterpret_cast<double*>(smraw + so.q);
+  double* As = reinterpret_cast<double*>(smraw + so.ainv);
+  int* ys = reinterpret_cast<int*>(smraw + so.ys);
+  int* gx = reinterpret_cast<int*>(smraw + so.gx);
+  int* gl = reinterpret_cast<int*>(smraw + so.gl);
+  int* goff = reinterpret_cast<int*>(smraw + so.goff);
+  const int warp = tid >> 5, lane = tid & 31;
+  constexpr int kWarps = kBclThreads / 32;
+
+  // rows of Ainv this CTA owns: one bulk copy global -> shared, completion on an mbarrier
+  const int rows_per = (B + CL - 1) / CL;
+  const int r0 = min(B, rank * rows_per), r1 = min(B, r0 + rows_per);
+  const bool bulk = ainv_in_smem && r1 > r0;
+  const unsigned bar = (unsigned)__cvta_generic_to_shared(smraw + so.bar);
+  if (bulk && tid == 0) {
+    const unsigned bytes = (unsigned)(r1 - r0) * (unsigned)Bs * 8u;
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(As);
+    const double* src = g.ainv + (size_t)r0 * Bs;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+  }
+  for (int i = tid; i < nx; i += kBclThreads) twx[i] = g.twxd[i];
+  for (int i = tid; i < ny; i += kBclThreads) twy[i] = g.twyd[i];
+  for (int i = tid; i < B; i += kBclThreads) { ys[i] = g.pad_y[i]; vpad[i] = g.pad_pot[i]; }
+  for (int i = tid; i < G; i += kBclThreads) { gx[i] = g.grp_x[i]; gl[i] = g.grp_layer[i]; }
+  for (int i = tid; i <= G; i += kBclThreads) goff[i] = g.grp_off[i];
+
+  // ---- phase 1: pad potentials of the free charge, groups [gbeg, gbeg + ng) ------------------------
+  {
+    const int gpc = (G + CL - 1) / CL;
+    const int gbeg = min(G, rank * gpc), ng = min(G, gbeg + gpc) - gbeg;
+    const int KC = so.kc, per = (nx + KC - 1) / KC;
+    double2* part = work;                               // [ng][KC][y2]
+    double2* tl = work + (size_t)so.gpc * KC * y2;      // [ng][y2]
+    const double2* __restrict__ plb = emit ? g.pl_e : g.pl;
+    // the first loads of pl need no table: the layer of group gbeg follows from the parameter space
+    constexpr int kPre = 4;                             // kx values held in registers
+    const bool one_pass = (KC * y2 <= kBclThreads) && per <= kPre && ng > 0;
+    double2 pre[kPre];
+    int pre_layer = 0;
+#pragma unroll
+    for (int l = 1; l < kMaxLayers; ++l) pre_layer += (l < L && g.lgoff[l] <= gbeg) ? 1 : 0;
+    if (one_pass && tid < KC * y2) {
+      const int ky = tid % y2, ch = tid / y2, k0 = min(nx, ch * per);
+#pragma unroll
+      for (int r = 0; r < kPre; ++r)
+        pre[r] = (k0 + r < nx && r < per) ? plb[((size_t)pre_layer * nx + k0 + r) * y2 + ky] : make_double2(0.0, 0.0);
+    }
+    WT_STAMP(1);
+    __syncthreads();
+    WT_STAMP(2);
+    for (int i = tid; i < KC * y2; i += kBclThreads) {
+      const int ky = i % y2, ch = i / y2;
+      const int k0 = min(nx, ch * per), k1 = min(nx, k0 + per);
+      for (int gi = 0; gi < ng; ++gi) {
+        const int x = gx[gbeg + gi], l = gl[gbeg + gi];
+        int idx = modx(k0 * x);
+        double2 s = make_double2(0.0, 0.0);
+        if (one_pass && l == pre_layer) {
+#pragma unroll
+          for (int r = 0; r < kPre; ++r) {
+            if (k0 + r < k1) {
+              double2 w = twx[idx];
+              w.y = -w.y;                               // e^{+i kx x}
+              const double2 p = dmul(pre[r], w);
+              s.x += p.x; s.y += p.y;
+              idx += x; if (idx >= nx) idx -= nx;
+            }
+          }
+        } else {
+          const double2* __restrict__ pl = plb + (size_t)l * nx * y2 + ky;
+          for (int kx = k0; kx < k1; ++kx) {
+            double2 w = twx[idx];
+            w.y = -w.y;
+            const double2 p = dmul(pl[(size_t)kx * y2], w);
+            s.x += p.x; s.y += p.y;
+            idx += x; if (idx >= nx) idx -= nx;
+          }
+        }
+        part[((size_t)gi * KC + ch) * y2 + ky] = s;
+      }
+    }
+    __syncthreads();
+    WT_STAMP(3);
+    for (int i = tid; i < ng * y2; i += kBclThreads) {
+      const int gi = i / y2, ky = i - gi * y2;
+      const double2* __restrict__ pp = part + (size_t)gi * KC * y2 + ky;
+      double2 s = make_double2(0.0, 0.0);
+#pragma unroll 8
+      for (int ch = 0; ch < KC; ++ch) { const double2 p = pp[ch * y2]; s.x += p.x; s.y += p.y; }
+      const double wgt = (ky == 0) ? 1.0 : 2.0;         // Hermitian half spectrum along y
+      tl[i] = make_double2(wgt * s.x, wgt * s.y);
+    }
+    __syncthreads();
+    WT_STAMP(4);
+    cluster.barrier_wait();                             // every CTA of the cluster is running
+    const int pbeg = goff[gbeg], pend = goff[gbeg + ng];
+    for (int p = pbeg + warp; p < pend; p += kWarps) {
+      int gi = 0;
+      while (goff[gbeg + gi + 1] <= p) ++gi;
+      const int y = ys[p];
+      double s = 0.0;
+      for (int ky = lane; ky < y2; ky += 32) {
+        const double2 w = twy[mody(ky * y)];            // Re(T e^{+i ky y}) = T.x w.x + T.y w.y, w = e^{-i ky y}
+        const double2 t = tl[gi * y2 + ky];
+        s += t.x * w.x + t.y * w.y;
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      if (lane < CL) cluster.map_shared_rank(rhs, lane)[p] = flag * vpad[p] - s;
+    }
+  }
+  WT_STAMP(5);
+  if (bulk) {                                           // the slice of Ainv has landed
+    unsigned done = 0;
+    while (!done) {
+      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                   : "=r"(done) : "r"(bar), "r"(0u) : "memory");
+    }
+  }
+  WT_STAMP(6);
+  cluster.sync();
+  WT_STAMP(7);
+
+  // ---- phase 2: Q' = Ainv rhs, rows [r0, r1) ---------------------------------------------------------
+  for (int row = r0 + warp; row < r1; row += kWarps) {
+    const double* __restrict__ a = ainv_in_smem ? As + (size_t)(row - r0) * Bs : g.ainv + (size_t)row * Bs;
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    int jj = lane;
+    for (; jj + 96 < B; jj += 128) {
+      s0 += a[jj] * rhs[jj]; s1 += a[jj + 32] * rhs[jj + 32];
+      s2 += a[jj + 64] * rhs[jj + 64]; s3 += a[jj + 96] * rhs[jj + 96];
+    }
+    for (; jj < B; jj += 32) s0 += a[jj] * rhs[jj];
+    double s = (s0 + s1) + (s2 + s3);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane < CL) cluster.map_shared_rank(qs, lane)[row] = s;
+  }
+  WT_STAMP(8);
+  cluster.sync();
+  WT_STAMP(9);
+
+  // ---- phase 3: spectrum of the boundary charges, rows (l, kx) in [rw0, rw1) -------------------------
+  {
+    const int n_rows = L * nx, rpc = (n_rows + CL - 1) / CL;
+    const int rw0 = min(n_rows, rank * rpc), rw1 = min(n_rows, rw0 + rpc);
+    if (rw0 < rw1) {
+      const int l0 = rw0 / nx, l1 = (rw1 - 1) / nx;
+      const int ga = g.lgoff[l0], gz = g.lgoff[l1 + 1];
+      double2* u = work;                                // [G][y2], groups [ga, gz) filled
+      for (int i = ga * y2 + tid; i < gz * y2; i += kBclThreads) {
+        const int grp = i / y2, ky = i - grp * y2;
+        double2 s0 = make_double2(0.0, 0.0), s1 = make_double2(0.0, 0.0);
+        int p = goff[grp];
+        const int pe = goff[grp + 1];
+        for (; p + 1 < pe; p += 2) {
+          const double2 w0 = twy[mody(ky * ys[p])], w1 = twy[mody(ky * ys[p + 1])];
+          const double q0 = qs[p], q1 = qs[p + 1];
+          s0.x += q0 * w0.x; s0.y += q0 * w0.y;
+          s1.x += q1 * w1.x; s1.y += q1 * w1.y;
+        }
+        if (p < pe) {
+          const double2 w0 = twy[mody(ky * ys[p])];
+          const double q0 = qs[p];
+          s0.x += q0 * w0.x; s0.y += q0 * w0.y;
+        }
+        u[i] = make_double2(s0.x + s1.x, s0.y + s1.y);
+      }
+      // wtab[row - rw0][grp] = e^{-i kx x_grp} for the groups of the row's layer
+      for (int i = tid; i < (rw1 - rw0) * G; i += kBclThreads) {
+        const int r = i / G, grp = i - r * G;
+        const int row = rw0 + r, l = row / nx, kx = row - l * nx;
+        if (grp >= g.lgoff[l] && grp < g.lgoff[l + 1]) wtab[i] = twx[modx(kx * gx[grp])];
+      }
+      WT_STAMP(10);
+      __syncthreads();
+      WT_STAMP(11);
+      for (int i = rw0 * y2 + tid; i < rw1 * y2; i += kBclThreads) {
+        const int ky = i % y2, row = i / y2, l = row / nx, kx = row - l * nx;
+        const double2* __restrict__ wt_ = wtab + (size_t)(row - rw0) * G;
+        double2 a0 = make_double2(0.0, 0.0), a1 = make_double2(0.0, 0.0);
+        int grp = g.lgoff[l];
+        const int ge = g.lgoff[l + 1];
+        for (; grp + 1 < ge; grp += 2) {
+          const double2 p0 = dmul(u[grp * y2 + ky], wt_[grp]), p1 = dmul(u[(grp + 1) * y2 + ky], wt_[grp + 1]);
+          a0.x += p0.x; a0.y += p0.y; a1.x += p1.x; a1.y += p1.y;
+        }
+        if (grp < ge) { const double2 p0 = dmul(u[grp * y2 + ky], wt_[grp]); a0.x += p0.x; a0.y += p0.y; }
+        double2 a = make_double2(a0.x + a1.x, a0.y + a1.y);
+        if (kx == nx / 2) a = make_double2(0.0, 0.0);   // removed Nyquist plane (R11)
+        g.qh[i] = make_float2((float)(a.x * gd.inv_n), (float)(a.y * gd.inv_n));
+      }
+    }
+  }
+  WT_STAMP(12);
+#undef WT_STAMP
 }
 
 }  // namespace wt

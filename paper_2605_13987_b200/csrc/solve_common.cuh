@@ -14,6 +14,7 @@ struct GridDev {
   int nx, ny, nz, y2, nt, ty, n_tiles;   // generic k_spectral: ty lines per CTA, n_tiles = nx * (y2/ty)
   double inv_n;
   const int* step;                        // device counter: index n of the output step being produced
+  long long* stamps;                      // debug (WTIDE_STAMPS=1): [16 ranks][16] clock stamps of the boundary kernel, else NULL
 };
 
 // One geometry of the lock-step batch.  Passed BY VALUE inside GeomBatch (kernel parameter space =
@@ -26,7 +27,7 @@ struct GeomDev {
   const float* sdt;          // [256]  s * dt_int of id
   const float* gt;           // [kx][dz][ky] mixed-space fundamental solution
   const float* gzt;          //              and its -d/dz
-  const double* ainv;        // [B][B] in group order
+  const double* ainv;        // [B][Bs] in group order, row stride Bs = B rounded up to even (16-byte rows)
   const double* pad_pot;     // [B]
   const int* pad_y;          // [B]
   const int* grp_x;          // [G]
@@ -48,7 +49,8 @@ struct GeomDev {
   float* stage;                        // [TB][3][z][..] staging of H for the time-innermost table write
   float* H;
   int layers[kMaxLayers];
-  int B, L, G, n_sub;
+  int lgoff[kMaxLayers + 1];           // copy of layer_goff in the parameter space
+  int B, Bs, L, G, n_sub;
   float inv_dt;
 };
 
