@@ -29,6 +29,7 @@
 #include <cstdlib>
 #include <map>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "geometry.h"
@@ -137,6 +138,28 @@ cudaError_t upload(char* base, size_t off, const std::vector<T>& v, cudaStream_t
     }                                                                                         \
   } while (0)
 
+// One launch: optional thread-block cluster along x, optional programmatic dependent launch (PDL).
+template <typename... KArgs, typename... Args>
+cudaError_t launch(void (*fn)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, bool pdl, int cluster,
+                   Args&&... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[2];
+  int n = 0;
+  if (cluster > 1) {
+    at[n].id = cudaLaunchAttributeClusterDimension;
+    at[n].val.clusterDim.x = cluster; at[n].val.clusterDim.y = 1; at[n].val.clusterDim.z = 1;
+    ++n;
+  }
+  if (pdl) {
+    at[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[n].val.programmaticStreamSerializationAllowed = 1;
+    ++n;
+  }
+  cfg.attrs = at; cfg.numAttrs = n;
+  return cudaLaunchKernelEx(&cfg, fn, std::forward<Args>(args)...);
+}
+
 // ---- kernel selection ---------------------------------------------------------------------------
 using PlaneFn = void (*)(const GeomBatch, GridDev, int);
 using LineFn = void (*)(const GeomBatch, GridDev, int, int);
@@ -174,8 +197,26 @@ void set_line_lt(Plan& p, int nx, int y2) {
   p.line_fast = true;
   p.ty = TYL;
 }
+template <int NZ, int E, int TYL, int LT>
+void set_line2_lt(Plan& p, int nx, int y2) {
+  using C = PencilCfg<NZ, E, TYL>;
+  p.line_step = k_pencil2<NZ, E, TYL, LT, true, false>;
+  p.line_init = k_pencil2<NZ, E, TYL, LT, false, false>;
+  p.line_delta = k_pencil2<NZ, E, TYL, LT, false, true>;
+  p.line_grid = dim3(nx * (y2 / TYL));
+  p.line_block = dim3(2 * C::THREADS);
+  p.line_smem = (size_t)2 * C::FIELD * sizeof(float2) + (size_t)2 * NZ * TYL * sizeof(float2) +
+                (size_t)LT * TYL * 2 * C::T * sizeof(double2);
+  p.line_fast = true;
+  p.ty = TYL;
+}
 template <int NZ, int E, int TYL>
 void set_line(Plan& p, int nx, int y2, int L) {
+  if (!env_flag("WTIDE_PENCIL1")) {
+    if (L <= 2) set_line2_lt<NZ, E, TYL, 2>(p, nx, y2);
+    else set_line2_lt<NZ, E, TYL, kMaxLayers>(p, nx, y2);
+    return;
+  }
   if (L <= 2) set_line_lt<NZ, E, TYL, 2>(p, nx, y2);
   else set_line_lt<NZ, E, TYL, kMaxLayers>(p, nx, y2);
 }
@@ -260,16 +301,23 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   const size_t sm_tr = (size_t)kStageSlots * 3 * std::max(nx, ny) * sizeof(float);
   // boundary adjust: one cluster launch per substep for small pad sets (16 CTAs where the device can
   // co-schedule the non-portable size, else 8), three grid-wide launches otherwise
-  const bool pow2 = (nx & (nx - 1)) == 0 && (ny & (ny - 1)) == 0;
-  const void* bnd_fn = pow2 ? (const void*)k_boundary_cluster<true> : (const void*)k_boundary_cluster<false>;
+  using BndFastFn = void (*)(const GeomBatch, GridDev, const BndClSmem, int, int, double);
+  BndFastFn bnd_fast = nullptr;
+  if (nx == ny && !env_flag("WTIDE_GENERIC")) {
+    if (nx == 32) bnd_fast = k_boundary_fast<5, 4>;
+    else if (nx == 64) bnd_fast = k_boundary_fast<6, 5>;
+    else if (nx == 128) bnd_fast = k_boundary_fast<7, 6>;
+  }
+  const void* bnd_fn = bnd_fast ? (const void*)bnd_fast : (const void*)k_boundary_cluster<false>;
+  const int bnd_threads = bnd_fast ? kBfThreads : kBclThreads;
   const int maxBs = (maxB + 1) & ~1;
   int bnd_cl = 8;
   BndClSmem bcl;
   int ainv_in_smem = 1;
   auto size_cluster = [&](int cl) {
     bnd_cl = cl; ainv_in_smem = 1;
-    bcl = bnd_cl_smem(nx, ny, kMaxLayers, maxG, maxB, maxBs, cl, true);
-    if (bcl.total > 200 * 1024) { bcl = bnd_cl_smem(nx, ny, kMaxLayers, maxG, maxB, maxBs, cl, false); ainv_in_smem = 0; }
+    bcl = bnd_cl_smem(nx, ny, kMaxLayers, maxG, maxB, maxBs, cl, true, bnd_threads);
+    if (bcl.total > 200 * 1024) { bcl = bnd_cl_smem(nx, ny, kMaxLayers, maxG, maxB, maxBs, cl, false, bnd_threads); ainv_in_smem = 0; }
   };
   size_cluster(16);
   bool bnd_cluster = maxB > 0 && maxB <= 640 && !env_flag("WTIDE_SPLIT_BOUNDARY");
@@ -279,7 +327,7 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
                 cudaFuncSetAttribute(bnd_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bcl.total) == cudaSuccess;
     if (ok16) {
       cudaLaunchConfig_t q = {};
-      q.gridDim = dim3(16, 1); q.blockDim = dim3(kBclThreads); q.dynamicSmemBytes = bcl.total;
+      q.gridDim = dim3(16, 1); q.blockDim = dim3(bnd_threads); q.dynamicSmemBytes = bcl.total;
       cudaLaunchAttribute at[1];
       at[0].id = cudaLaunchAttributeClusterDimension;
       at[0].val.clusterDim.x = 16; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
@@ -392,6 +440,7 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   const int bnd_rows = (maxB + kBndThreads / 32 - 1) / (kBndThreads / 32);
 
   const int dbg_skip = std::getenv("WTIDE_DBG_SKIP") ? std::atoi(std::getenv("WTIDE_DBG_SKIP")) : 0;
+  const bool pdl = !env_flag("WTIDE_NO_PDL");
   long long launches = 0;
   cudaError_t launch_err = cudaSuccess;
   auto note = [&](cudaError_t e) { if (e != cudaSuccess && launch_err == cudaSuccess) launch_err = e; };
@@ -402,19 +451,14 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
       const int nb = batch_n[bi];
       if (bnd_cluster) {
         ++launches;
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(bnd_cl, nb); cfg.blockDim = dim3(kBclThreads); cfg.dynamicSmemBytes = bcl.total; cfg.stream = st;
-        cudaLaunchAttribute at[1];
-        at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = bnd_cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
-        cfg.attrs = at; cfg.numAttrs = 1;
-        if (pow2) note(cudaLaunchKernelEx(&cfg, k_boundary_cluster<true>, gb, gd, maxG, maxB, maxBs, ainv_in_smem, s, emit, flag));
-        else note(cudaLaunchKernelEx(&cfg, k_boundary_cluster<false>, gb, gd, maxG, maxB, maxBs, ainv_in_smem, s, emit, flag));
+        if (bnd_fast) note(launch(bnd_fast, dim3(bnd_cl, nb), dim3(bnd_threads), bcl.total, st, pdl, bnd_cl, gb, gd, bcl, s, emit, flag));
+        else note(launch(k_boundary_cluster<false>, dim3(bnd_cl, nb), dim3(bnd_threads), bcl.total, st, pdl, bnd_cl, gb, gd, maxG,
+                         maxB, maxBs, ainv_in_smem, s, emit, flag));
       } else {
         launches += 3;
-        k_boundary<1><<<dim3(std::max(1, maxG), nb), kBndThreads, bsm.total, st>>>(gb, gd, maxGL, s, emit, flag);
-        k_boundary<2><<<dim3(std::max(1, bnd_rows), nb), kBndThreads, bsm.total, st>>>(gb, gd, maxGL, s, emit, flag);
-        k_boundary<3><<<dim3(bnd_units3, nb), kBndThreads, bsm.total, st>>>(gb, gd, maxGL, s, emit, flag);
+        note(launch(k_boundary<1>, dim3(std::max(1, maxG), nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
+        note(launch(k_boundary<2>, dim3(std::max(1, bnd_rows), nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
+        note(launch(k_boundary<3>, dim3(bnd_units3, nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
       }
     }
   };
@@ -422,13 +466,13 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     for (int bi = 0; bi < n_batches; ++bi) {
       ++launches;
       const dim3 grid = plan.plane_fast ? dim3(nz, 3, batch_n[bi]) : dim3(nz, batch_n[bi]);
-      fn<<<grid, plan.plane_block, plan.plane_smem, st>>>(batches[bi], gd, s);
+      note(launch(fn, grid, plan.plane_block, plan.plane_smem, st, pdl, 1, batches[bi], gd, s));
     }
   };
   auto line = [&](LineFn fn, int s, int emit) {
     for (int bi = 0; bi < n_batches; ++bi) {
       ++launches;
-      fn<<<dim3(plan.line_grid.x, batch_n[bi]), plan.line_block, plan.line_smem, st>>>(batches[bi], gd, s, emit);
+      note(launch(fn, dim3(plan.line_grid.x, batch_n[bi]), plan.line_block, plan.line_smem, st, pdl, 1, batches[bi], gd, s, emit));
     }
   };
   auto emit_step = [&](bool first) {
@@ -439,11 +483,11 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
     plane(plan.plane_emit, 0);
     for (int bi = 0; bi < n_batches; ++bi) {
       ++launches;
-      if (plan.plane_fast) k_transpose<true><<<dim3(n_tr, batch_n[bi]), 256, sm_tr, st>>>(batches[bi], gd);
-      else                 k_transpose<false><<<dim3(n_tr, batch_n[bi]), 256, sm_tr, st>>>(batches[bi], gd);
+      if (plan.plane_fast) note(launch(k_transpose<true>, dim3(n_tr, batch_n[bi]), dim3(256), sm_tr, st, pdl, 1, batches[bi], gd));
+      else                 note(launch(k_transpose<false>, dim3(n_tr, batch_n[bi]), dim3(256), sm_tr, st, pdl, 1, batches[bi], gd));
     }
     ++launches;
-    k_advance<<<1, 1, 0, st>>>(dstep);
+    note(launch(k_advance, dim3(1), dim3(1), 0, st, pdl, 1, dstep));
   };
   auto output_step = [&]() {
     for (int s = 0; s < max_sub; ++s) {

@@ -21,6 +21,9 @@
 
 namespace wt {
 
+// debug (WTIDE_STAMPS=1): clock stamps of thread 0 of each CTA of geometry 0
+#define WT_STAMP(k) do { if (gd.stamps && threadIdx.x == 0 && blockIdx.y == 0) gd.stamps[blockIdx.x * 16 + (k)] = clock64(); } while (0)
+
 constexpr int kBndCluster = 8;
 constexpr int kBndThreads = 512;
 constexpr int kBndChunks = 16;   // kx range split of phase 1
@@ -48,8 +51,10 @@ __host__ __device__ inline BndSmem bnd_smem(int nx, int ny, int max_groups_per_l
 template <int PHASE>
 __global__ void __launch_bounds__(kBndThreads)
 k_boundary(const __grid_constant__ GeomBatch gb, GridDev gd, int max_gl, int substep, int emit, double flag) {
+  pdl_trigger();
   const GeomDev& g = gb.g[blockIdx.y];
-  if (substep >= g.n_sub || g.B == 0) return;       // uniform over the geometry's CTAs
+  if (substep >= g.n_sub || g.B == 0) { pdl_wait(); return; }   // uniform over the geometry's CTAs
+  pdl_wait();
   const int nx = gd.nx, ny = gd.ny, y2 = gd.y2, tid = threadIdx.x;
   const int cta = blockIdx.x, n_cta = gridDim.x;
   const int B = g.B;
@@ -190,13 +195,16 @@ constexpr int kBclThreads = 1024;
 
 struct BndClSmem {
   size_t bar, twx, twy, vpad, rhs, q, work, wtab, ys, gx, gl, goff, ainv, total;
-  int kc, gpc, rows, rpc;
+  int kc, gpc, rows, rpc, lcl, in_smem;
 };
-__host__ __device__ inline BndClSmem bnd_cl_smem(int nx, int ny, int L, int G, int B, int Bs, int CL, bool ainv_in_smem) {
+__host__ __device__ inline BndClSmem bnd_cl_smem(int nx, int ny, int L, int G, int B, int Bs, int CL, bool ainv_in_smem,
+                                                 int threads = kBclThreads) {
   BndClSmem s;
   const int y2 = ny / 2;
   const int Gp = G > 0 ? G : 1, Bp = B > 0 ? B : 1, Lp = L > 0 ? L : 1;
-  s.kc = kBclThreads / y2 < 1 ? 1 : (kBclThreads / y2 > nx ? nx : kBclThreads / y2);
+  s.lcl = CL == 16 ? 4 : 3;
+  s.in_smem = ainv_in_smem ? 1 : 0;
+  s.kc = threads / y2 < 1 ? 1 : (threads / y2 > nx ? nx : threads / y2);
   s.gpc = (Gp + CL - 1) / CL;
   s.rows = (Bp + CL - 1) / CL;
   s.rpc = (Lp * nx + CL - 1) / CL;
@@ -204,7 +212,7 @@ __host__ __device__ inline BndClSmem bnd_cl_smem(int nx, int ny, int L, int G, i
   s.bar = p; p += 16;
   s.twx = p; p += (size_t)nx * 16;
   s.twy = p; p += (size_t)ny * 16;
-  const size_t w1 = (size_t)(s.kc + 1) * s.gpc * y2 * 16, w3 = (size_t)Gp * y2 * 16;
+  const size_t w1 = (size_t)(s.kc + 1) * s.gpc * y2 * 16, w3 = ((size_t)Gp + 4 * (size_t)s.rpc) * y2 * 16;
   s.work = p; p += (w1 > w3 ? w1 : w3);
   s.wtab = p; p += (size_t)s.rpc * Gp * 16;
   s.ainv = p; p += ainv_in_smem ? (size_t)s.rows * Bs * 8 : 0;
@@ -224,11 +232,12 @@ __global__ void __launch_bounds__(kBclThreads, 1)
 k_boundary_cluster(const __grid_constant__ GeomBatch gb, GridDev gd, int max_g, int max_b, int max_bs, int ainv_in_smem,
                    int substep, int emit, double flag) {
   namespace cg = cooperative_groups;
+  pdl_trigger();
   const GeomDev& g = gb.g[blockIdx.y];
-  if (substep >= g.n_sub || g.B == 0) return;       // uniform over the cluster
+  if (substep >= g.n_sub || g.B == 0) { pdl_wait(); return; }   // uniform over the cluster
+  pdl_wait();
   cg::cluster_group cluster = cg::this_cluster();
   cluster.barrier_arrive();                         // (waited for before the first remote store)
-#define WT_STAMP(k) do { if (gd.stamps && threadIdx.x == 0 && blockIdx.y == 0) gd.stamps[blockIdx.x * 16 + (k)] = clock64(); } while (0)
   WT_STAMP(0);
   const int CL = gridDim.x;                         // grid.x == cluster size
   const int rank = blockIdx.x;
@@ -443,7 +452,285 @@ k_boundary_cluster(const __grid_constant__ GeomBatch gb, GridDev gd, int max_g, 
     }
   }
   WT_STAMP(12);
-#undef WT_STAMP
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// k_boundary_fast<LNX, LY2>: k_boundary_cluster for nx = 2^LNX, ny = 2^(LY2+1) with every index
+// operation a shift or a mask and the shared-memory layout computed on the host (the generic kernel
+// spends most of its issue slots on integer division).  512 threads.
+// ------------------------------------------------------------------------------------------------
+constexpr int kBfThreads = 512;
+
+template <int LNX, int LY2>
+__global__ void __launch_bounds__(kBfThreads, 1)
+k_boundary_fast(const __grid_constant__ GeomBatch gb, GridDev gd, const __grid_constant__ BndClSmem so, int substep, int emit,
+                double flag) {
+  namespace cg = cooperative_groups;
+  constexpr int NX = 1 << LNX, Y2 = 1 << LY2, NY = 2 * Y2;
+  constexpr int KC = (kBfThreads / Y2 > NX) ? NX : kBfThreads / Y2;   // kx chunks of phase 1
+  constexpr int PER = NX / KC;
+  constexpr int kWarps = kBfThreads / 32;
+  static_assert(KC * Y2 <= kBfThreads && NX <= kBfThreads && NY <= kBfThreads, "sizes");
+  pdl_trigger();
+  const GeomDev& g = gb.g[blockIdx.y];
+  if (substep >= g.n_sub || g.B == 0) { pdl_wait(); return; }   // uniform over the cluster
+  cg::cluster_group cluster = cg::this_cluster();
+  cluster.barrier_arrive();                         // (waited for before the first remote store)
+  WT_STAMP(0);
+  const int CL = gridDim.x, lcl = so.lcl;           // grid.x == cluster size = 2^lcl
+  const int rank = blockIdx.x, tid = threadIdx.x;
+  const int warp = tid >> 5, lane = tid & 31;
+  const int B = g.B, Bs = g.Bs, G = g.G, L = g.L;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  double2* twx = reinterpret_cast<double2*>(smraw + so.twx);    // e^{-2 pi i k/nx}
+  double2* twy = reinterpret_cast<double2*>(smraw + so.twy);
+  double2* work = reinterpret_cast<double2*>(smraw + so.work);
+  double2* wtab = reinterpret_cast<double2*>(smraw + so.wtab);
+  double* vpad = reinterpret_cast<double*>(smraw + so.vpad);
+  double* rhs = reinterpret_cast<double*>(smraw + so.rhs);
+  double* qs = reinterpret_cast<double*>(smraw + so.q);
+  double* As = reinterpret_cast<double*>(smraw + so.ainv);
+  int* ys = reinterpret_cast<int*>(smraw + so.ys);
+  int* gx = reinterpret_cast<int*>(smraw + so.gx);
+  int* gl = reinterpret_cast<int*>(smraw + so.gl);
+  int* goff = reinterpret_cast<int*>(smraw + so.goff);
+
+  // rows of Ainv this CTA owns: one bulk copy global -> shared, completion on an mbarrier
+  const int rows_per = (B + CL - 1) >> lcl;
+  const int r0 = min(B, rank * rows_per), r1 = min(B, r0 + rows_per);
+  const bool bulk = so.in_smem && r1 > r0;
+  const unsigned bar = (unsigned)__cvta_generic_to_shared(smraw + so.bar);
+  if (bulk && tid == 0) {
+    const unsigned bytes = (unsigned)(r1 - r0) * (unsigned)Bs * 8u;
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(As);
+    const double* src = g.ainv + (size_t)r0 * Bs;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+  }
+  if (tid < NX) twx[tid] = g.twxd[tid];
+  if (tid < NY) twy[tid] = g.twyd[tid];
+  for (int i = tid; i < B; i += kBfThreads) { ys[i] = g.pad_y[i]; vpad[i] = g.pad_pot[i]; }
+  for (int i = tid; i < G; i += kBfThreads) { gx[i] = g.grp_x[i]; gl[i] = g.grp_layer[i]; }
+  for (int i = tid; i <= G; i += kBfThreads) goff[i] = g.grp_off[i];
+
+  // rows (l, kx) of Q^ this CTA owns in phase 3
+  const int n_rows = L << LNX, rpc = (n_rows + CL - 1) >> lcl;
+  const int rw0 = min(n_rows, rank * rpc), rw1 = min(n_rows, rw0 + rpc);
+  const int gpc = (G + CL - 1) >> lcl;
+
+  // ---- phase 1: pad potentials of the free charge, groups [gbeg, gbeg + ng) ------------------------
+  {
+    const int gbeg = min(G, rank * gpc), ng = min(G, gbeg + gpc) - gbeg;
+    double2* part = work;                               // [ng][KC][Y2]
+    double2* tl = work + (size_t)so.gpc * KC * Y2;      // [ng][Y2]
+    const double2* __restrict__ plb = emit ? g.pl_e : g.pl;
+    const int ky = tid & (Y2 - 1), ch = tid >> LY2, k0 = ch * PER;
+    const bool act = tid < KC * Y2;
+    // the first loads of pl need no table: the layer of group gbeg follows from the parameter space
+    constexpr int kPre = PER <= 4 ? PER : 1;
+    constexpr bool kUsePre = PER <= 4;
+    double2 pre[kPre];
+    int pre_layer = 0;
+#pragma unroll
+    for (int l = 1; l < kMaxLayers; ++l) pre_layer += (l < L && g.lgoff[l] <= gbeg) ? 1 : 0;
+    pdl_wait();                                         // pl is written by the z-line kernel
+    if (kUsePre && act && ng > 0) {
+#pragma unroll
+      for (int r = 0; r < kPre; ++r) pre[r] = plb[((size_t)pre_layer * NX + k0 + r) * Y2 + ky];
+    }
+    WT_STAMP(1);
+    __syncthreads();
+    WT_STAMP(2);
+    if (act) {
+      for (int gi = 0; gi < ng; ++gi) {
+        const int x = gx[gbeg + gi], l = gl[gbeg + gi];
+        int idx = (k0 * x) & (NX - 1);
+        double2 s = make_double2(0.0, 0.0);
+        if (kUsePre && l == pre_layer) {
+#pragma unroll
+          for (int r = 0; r < kPre; ++r) {
+            double2 w = twx[idx];
+            w.y = -w.y;                                 // e^{+i kx x}
+            const double2 p = dmul(pre[r], w);
+            s.x += p.x; s.y += p.y;
+            idx = (idx + x) & (NX - 1);
+          }
+        } else {
+          const double2* __restrict__ pl = plb + ((size_t)l * NX + k0) * Y2 + ky;
+#pragma unroll 4
+          for (int r = 0; r < PER; ++r) {
+            double2 w = twx[idx];
+            w.y = -w.y;
+            const double2 p = dmul(pl[(size_t)r * Y2], w);
+            s.x += p.x; s.y += p.y;
+            idx = (idx + x) & (NX - 1);
+          }
+        }
+        part[(gi * KC + ch) * Y2 + ky] = s;
+      }
+    }
+    // (independent of the charges) wtab[row - rw0][grp] = e^{-i kx x_grp} for phase 3
+    for (int r = warp; r < rw1 - rw0; r += kWarps) {
+      const int row = rw0 + r, l = row >> LNX, kx = row & (NX - 1);
+      for (int grp = g.lgoff[l] + lane; grp < g.lgoff[l + 1]; grp += 32) wtab[r * G + grp] = twx[(kx * gx[grp]) & (NX - 1)];
+    }
+    __syncthreads();
+    WT_STAMP(3);
+    for (int i = tid; i < ng * Y2; i += kBfThreads) {
+      const int gi = i >> LY2, kk = i & (Y2 - 1);
+      const double2* __restrict__ pp = part + gi * KC * Y2 + kk;
+      double2 s0 = make_double2(0.0, 0.0), s1 = make_double2(0.0, 0.0);
+#pragma unroll
+      for (int c = 0; c < KC; c += 2) {
+        const double2 p = pp[c * Y2];
+        s0.x += p.x; s0.y += p.y;
+        if (c + 1 < KC) { const double2 q = pp[(c + 1) * Y2]; s1.x += q.x; s1.y += q.y; }
+      }
+      const double wgt = (kk == 0) ? 1.0 : 2.0;         // Hermitian half spectrum along y
+      tl[i] = make_double2(wgt * (s0.x + s1.x), wgt * (s0.y + s1.y));
+    }
+    __syncthreads();
+    WT_STAMP(4);
+    cluster.barrier_wait();                             // every CTA of the cluster is running
+    const int pbeg = goff[gbeg], pend = goff[gbeg + ng];
+    for (int p = pbeg + warp; p < pend; p += kWarps) {
+      int gi = 0;
+      while (goff[gbeg + gi + 1] <= p) ++gi;
+      const int y = ys[p];
+      double s = 0.0;
+#pragma unroll
+      for (int kk = lane; kk < Y2; kk += 32) {
+        const double2 w = twy[(kk * y) & (NY - 1)];     // Re(T e^{+i ky y}) = T.x w.x + T.y w.y, w = e^{-i ky y}
+        const double2 t = tl[gi * Y2 + kk];
+        s += t.x * w.x + t.y * w.y;
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+      if (lane == 0) rhs[p] = flag * vpad[p] - s;
+    }
+  }
+  WT_STAMP(5);
+  if (bulk) {                                           // the slice of Ainv has landed
+    unsigned done = 0;
+    while (!done) {
+      asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                   : "=r"(done) : "r"(bar), "r"(0u) : "memory");
+    }
+  }
+  WT_STAMP(6);
+  cluster.sync();
+  WT_STAMP(7);
+  // pull the other CTAs' rhs values (one warp per remote CTA, coalesced DSMEM reads)
+  for (int r = warp; r < CL; r += kWarps) {
+    if (r == rank) continue;
+    const int gb0 = min(G, r * gpc), gb1 = min(G, gb0 + gpc);
+    const double* __restrict__ remote = cluster.map_shared_rank(rhs, r);
+    for (int p = goff[gb0] + lane; p < goff[gb1]; p += 32) rhs[p] = remote[p];
+  }
+  __syncthreads();
+
+  // ---- phase 2: Q' = Ainv rhs, rows [r0, r1) ---------------------------------------------------------
+  for (int row = r0 + warp; row < r1; row += kWarps) {
+    double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+    int jj = lane;
+    if (so.in_smem) {
+      const double* __restrict__ a = As + (row - r0) * Bs;
+      for (; jj + 96 < B; jj += 128) {
+        s0 += a[jj] * rhs[jj]; s1 += a[jj + 32] * rhs[jj + 32];
+        s2 += a[jj + 64] * rhs[jj + 64]; s3 += a[jj + 96] * rhs[jj + 96];
+      }
+      for (; jj < B; jj += 32) s0 += a[jj] * rhs[jj];
+    } else {
+      const double* __restrict__ a = g.ainv + (size_t)row * Bs;
+      for (; jj + 96 < B; jj += 128) {
+        s0 += a[jj] * rhs[jj]; s1 += a[jj + 32] * rhs[jj + 32];
+        s2 += a[jj + 64] * rhs[jj + 64]; s3 += a[jj + 96] * rhs[jj + 96];
+      }
+      for (; jj < B; jj += 32) s0 += a[jj] * rhs[jj];
+    }
+    double s = (s0 + s1) + (s2 + s3);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) qs[row] = s;
+  }
+  WT_STAMP(8);
+  cluster.sync();
+  WT_STAMP(9);
+  for (int r = warp; r < CL; r += kWarps) {
+    if (r == rank) continue;
+    const int q0 = min(B, r * rows_per), q1 = min(B, q0 + rows_per);
+    const double* __restrict__ remote = cluster.map_shared_rank(qs, r);
+    for (int p = q0 + lane; p < q1; p += 32) qs[p] = remote[p];
+  }
+  cluster.barrier_arrive();                             // (no remote access after this point; waited for at exit)
+  __syncthreads();
+
+  // ---- phase 3: spectrum of the boundary charges, rows (l, kx) in [rw0, rw1) -------------------------
+  if (rw0 < rw1) {
+    const int l0 = rw0 >> LNX, l1 = (rw1 - 1) >> LNX;
+    const int ga = g.lgoff[l0], gz = g.lgoff[l1 + 1];
+    double2* u = work;                                  // [G][Y2], groups [ga, gz) filled
+    for (int i = ga * Y2 + tid; i < gz * Y2; i += kBfThreads) {
+      // u[grp][ky] = sum_p Q'_p e^{-i ky y_p}; along a run of consecutive y the phase advances by the
+      // fixed factor e^{-i ky} (one table lookup per run instead of one per pad)
+      const int grp = i >> LY2, kk = i & (Y2 - 1);
+      const double2 stepw = twy[kk];
+      double2 s = make_double2(0.0, 0.0), w = make_double2(1.0, 0.0);
+      int yprev = -2;
+      for (int p = goff[grp]; p < goff[grp + 1]; ++p) {
+        const int y = ys[p];
+        w = (y == yprev + 1) ? dmul(w, stepw) : twy[(kk * y) & (NY - 1)];
+        yprev = y;
+        const double q = qs[p];
+        s.x += q * w.x; s.y += q * w.y;
+      }
+      u[i] = s;
+    }
+    WT_STAMP(10);
+    __syncthreads();
+    WT_STAMP(11);
+    // Q^_l[kx][ky] = (1/N) sum_{g in l} u[g][ky] e^{-i kx x_g}: the group range is split over kSplit thread sets
+    const int n_out = (rw1 - rw0) * Y2;
+    int kSplit = 1;
+    while (kSplit < 4 && n_out * (kSplit * 2) <= kBfThreads) kSplit *= 2;
+    double2* red = work + (size_t)G * Y2;               // [kSplit][n_out]  (after u)
+    for (int i0 = 0; i0 < n_out; i0 += kBfThreads / kSplit) {
+      const int o = i0 + (tid % (kBfThreads / kSplit)), part_i = tid / (kBfThreads / kSplit);
+      double2 a0 = make_double2(0.0, 0.0), a1 = make_double2(0.0, 0.0);
+      if (o < n_out && part_i < kSplit) {
+        const int i = rw0 * Y2 + o;
+        const int kk = i & (Y2 - 1), row = i >> LY2, l = row >> LNX;
+        const double2* __restrict__ wt_ = wtab + (row - rw0) * G;
+        const double2* __restrict__ uu = u + kk;
+        const int gs = g.lgoff[l], ge = g.lgoff[l + 1];
+        const int per_part = (ge - gs + kSplit - 1) / kSplit;
+        int grp = gs + part_i * per_part;
+        const int gend = min(ge, grp + per_part);
+        for (; grp + 1 < gend; grp += 2) {
+          const double2 p0 = dmul(uu[grp * Y2], wt_[grp]), p1 = dmul(uu[(grp + 1) * Y2], wt_[grp + 1]);
+          a0.x += p0.x; a0.y += p0.y; a1.x += p1.x; a1.y += p1.y;
+        }
+        if (grp < gend) { const double2 p0 = dmul(uu[grp * Y2], wt_[grp]); a0.x += p0.x; a0.y += p0.y; }
+        red[part_i * n_out + o] = make_double2(a0.x + a1.x, a0.y + a1.y);
+      }
+      __syncthreads();
+      if (o < n_out && part_i == 0) {
+        const int i = rw0 * Y2 + o;
+        const int kx = (i >> LY2) & (NX - 1);
+        double2 a = red[o];
+        for (int k = 1; k < kSplit; ++k) { const double2 b = red[k * n_out + o]; a.x += b.x; a.y += b.y; }
+        if (kx == NX / 2) a = make_double2(0.0, 0.0);   // removed Nyquist plane (R11)
+        g.qh[i] = make_float2((float)(a.x * gd.inv_n), (float)(a.y * gd.inv_n));
+      }
+      __syncthreads();
+    }
+  }
+  WT_STAMP(12);
+  cluster.barrier_wait();
 }
 
 }  // namespace wt

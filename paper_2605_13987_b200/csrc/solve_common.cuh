@@ -56,6 +56,13 @@ struct GeomDev {
 
 struct GeomBatch { GeomDev g[kBatch]; };
 
+// Programmatic dependent launch (PDL): every kernel of wt_solve_H lets its successor start launching at
+// once (its CTAs fill SMs as ours drain and run their prologue, which reads static tables only) and
+// waits for the full completion of its predecessor before touching anything a kernel writes.
+// Both are no-ops when the kernel was launched without the PDL attribute.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 __device__ __forceinline__ double2 dmul(double2 a, double2 b) {
   return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
 }

@@ -37,8 +37,9 @@ __global__ void __launch_bounds__(N * N / (2 * E), (N <= 64) ? 4 : 1)
 k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
   using C = PlaneCfg<N>;
   constexpr int Y2 = C::Y2, T = N / E, SX = C::SX, SU = C::SU, BUF = C::BUF;
+  pdl_trigger();
   const GeomDev& g = gb.g[blockIdx.z];
-  if (substep >= g.n_sub) return;
+  if (substep >= g.n_sub) { pdl_wait(); return; }
   const int nz = gd.nz, z = blockIdx.x, comp = blockIdx.y;
   const int tid = threadIdx.x;
   const int ln = tid % Y2;     // line within the phase: ky (x-phases) or p2 (y-phases)
@@ -59,6 +60,7 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
     for (int r = 0; r < E; ++r) sid[r] = __ldg(st + ((j + T * r) * N + 2 * ln) / 2);
   }
 
+  pdl_wait();
   float2 X[E];
   // ---- load: V~ = V~_rho + sum_l Q^_l g~(z - z_l) (the boundary source, a4); E~ = -i kappa V~ ------------
   {
@@ -211,8 +213,9 @@ __global__ void __launch_bounds__(PencilCfg<NZ, E, TYL>::THREADS)
 k_pencil(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emit) {
   using C = PencilCfg<NZ, E, TYL>;
   constexpr int T = C::T, QS = C::QS, FIELD = C::FIELD;
+  pdl_trigger();
   const GeomDev& g = gb.g[blockIdx.y];
-  if (substep >= g.n_sub) return;
+  if (substep >= g.n_sub) { pdl_wait(); return; }
   const int nx = gd.nx, y2 = gd.y2;
   const int tiles = y2 / TYL;
   const int kx = blockIdx.x / tiles, ky0 = (blockIdx.x % tiles) * TYL;
@@ -228,6 +231,7 @@ k_pencil(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emit
   float2 w[E];
   load_twiddles<E>(w, g.twz, j);
   float2 A[E], Bf[E];                       // (D^ | V^), (J^z | -i kz V^)
+  pdl_wait();
 
   if constexpr (APPLY_J) {
     const float2* __restrict__ m0 = g.m0 + slab;
@@ -327,6 +331,143 @@ k_pencil(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emit
       oV[o] = A[r];
       oE[o] = Bf[r];
     }
+  }
+}
+
+
+// ------------------------------------------------------------------------------------------------
+// k_pencil2: the z-line kernel with ONE field per thread (twice the threads of k_pencil, half the
+// registers): threads (f = 0, line, j) transform D~ / V^, threads (f = 1, line, j) transform
+// J~z / -i kz V^.  The per-mode update needs both fields of a mode: after the forward transform the
+// spectra pass through a kz-indexed shared buffer, each thread updates E/2 modes of its line
+// in place (V^ and -i kz V^ overwrite D^ and J^z), and the inverse transforms read them back.
+// grid (nx * y2/TYL, n_geoms), block 2 * TYL * NZ/E.
+// dynamic smem: 2 fields * E * QS float2 (exchange) + 2 * NZ * TYL float2 (kz-indexed) + LT * TYL * 2T double2.
+// ------------------------------------------------------------------------------------------------
+template <int NZ, int E, int TYL, int LT, bool APPLY_J, bool DELTA>
+__global__ void __launch_bounds__(2 * PencilCfg<NZ, E, TYL>::THREADS, 2)
+k_pencil2(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emit) {
+  using C = PencilCfg<NZ, E, TYL>;
+  constexpr int T = C::T, QS = C::QS, FIELD = C::FIELD, HT = C::THREADS;   // HT threads per field
+  pdl_trigger();
+  const GeomDev& g = gb.g[blockIdx.y];
+  if (substep >= g.n_sub) { pdl_wait(); return; }
+  const int nx = gd.nx, y2 = gd.y2;
+  const int tiles = y2 / TYL;
+  const int kx = blockIdx.x / tiles, ky0 = (blockIdx.x % tiles) * TYL;
+  const int tid = threadIdx.x;
+  const int f = tid / HT, th = tid % HT;
+  const int line = th % TYL, j = th / TYL;
+  const int ky = ky0 + line;
+  const int L = g.L;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  float2* buf = reinterpret_cast<float2*>(smraw) + f * FIELD;                  // [2][E][QS]   exchange of this field
+  float2* kzb = reinterpret_cast<float2*>(smraw) + 2 * FIELD;                  // [2][NZ][TYL] kz-indexed spectra
+  double2* red = reinterpret_cast<double2*>(kzb + 2 * NZ * TYL);               // [LT][TYL][2T]
+  const size_t slab = (size_t)kx * NZ * y2 + ky;
+
+  float2 w[E];
+  load_twiddles<E>(w, g.twz, j);
+  float2 X[E];
+  pdl_wait();
+
+  if constexpr (APPLY_J) {
+    if (f == 0) {
+      const float2* __restrict__ m0 = g.m0 + slab;
+      const float2* __restrict__ m1 = g.m1 + slab;
+#pragma unroll
+      for (int r = 0; r < E; ++r) {
+        const size_t o = (size_t)(j + T * r) * y2;
+        const float2 a = m0[o], b = m1[o];
+        X[r] = make_float2(a.x + b.x, a.y + b.y);      // D~ = i kx J~x + i ky J~y
+      }
+    } else {
+      const float2* __restrict__ m2 = g.m2 + slab;
+#pragma unroll
+      for (int r = 0; r < E; ++r) X[r] = m2[(size_t)(j + T * r) * y2];
+    }
+    fft_stage1<E, false>(X, w);
+#pragma unroll
+    for (int q = 0; q < E; ++q) buf[q * QS + j * TYL + line] = X[q];
+    __syncthreads();
+    fft_stage2<E, T, false>(X, j, [&](int q, int jj) { return buf[q * QS + jj * TYL + line]; });
+    // X[p] = spectrum at kz = j + T p: into the kz-indexed buffer
+#pragma unroll
+    for (int p = 0; p < E; ++p) kzb[(f * NZ + j + T * p) * TYL + line] = X[p];
+    __syncthreads();
+  }
+
+  // ---- per-mode update (a7), potential from charge (a2), pad-layer sums (a3, fp64) ------------------------
+  // thread (f, line, j) owns the modes kz = j + T (2 i + f), i < E/2
+  {
+    double2 acc[LT];
+#pragma unroll
+    for (int l = 0; l < LT; ++l) acc[l] = make_double2(0.0, 0.0);
+    const double kxd = g.kxd[kx], kyd = g.kyd[ky];
+    const double kxy2 = kxd * kxd + kyd * kyd;
+    const bool ret_x = (kx != nx / 2);
+    double2* __restrict__ rh = g.rhat + slab;
+    double2* __restrict__ rp = g.rhat_prev + slab;
+#pragma unroll
+    for (int i = 0; i < E / 2; ++i) {
+      const int kz = j + T * (2 * i + f);
+      const size_t o = (size_t)kz * y2;
+      const bool ret = ret_x && (kz != NZ / 2);
+      const double kzd = g.kzd[kz];
+      double2 rr = rh[o];
+      if constexpr (APPLY_J) {
+        const float2 D = kzb[kz * TYL + line], J = kzb[(NZ + kz) * TYL + line];
+        const float kzf = (float)kzd;
+        rr.x -= (double)(D.x - kzf * J.y);
+        rr.y -= (double)(D.y + kzf * J.x);
+        if (!ret) rr = make_double2(0.0, 0.0);
+        rh[o] = rr;
+      }
+      double2 src = rr;
+      if constexpr (DELTA) {
+        const double2 p = rp[o];
+        src.x -= p.x; src.y -= p.y;
+        rp[o] = rr;
+      }
+      const double k2 = kxy2 + kzd * kzd;
+      const double gg = (ret && k2 > 0.0) ? gd.inv_n * fast_rcp(k2) : 0.0;
+      const double2 v = make_double2(src.x * gg, src.y * gg);
+      kzb[kz * TYL + line] = make_float2((float)v.x, (float)v.y);
+      kzb[(NZ + kz) * TYL + line] = make_float2((float)(kzd * v.y), (float)(-kzd * v.x));   // -i kz V^
+#pragma unroll
+      for (int l = 0; l < LT; ++l) {
+        if (l < L) {
+          double2 ww = g.twzd[(kz * g.layers[l]) & (NZ - 1)];
+          ww.y = -ww.y;                                                 // e^{+i kz z_l}
+          const double2 p = dmul(v, ww);
+          acc[l].x += p.x; acc[l].y += p.y;
+        }
+      }
+    }
+#pragma unroll
+    for (int l = 0; l < LT; ++l)
+      if (l < L) red[(l * TYL + line) * (2 * T) + f * T + j] = acc[l];
+  }
+  __syncthreads();
+  for (int i = tid; i < L * TYL; i += 2 * HT) {       // V~_rho(kx, z_l, ky) in fp64, fixed summation order
+    double2 s = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < 2 * T; ++k) { const double2 p = red[i * (2 * T) + k]; s.x += p.x; s.y += p.y; }
+    const int l = i / TYL, ln = i - l * TYL;
+    (emit ? g.pl_e : g.pl)[((size_t)l * nx + kx) * y2 + ky0 + ln] = s;
+  }
+  // ---- inverse z transform of this thread's field --------------------------------------------------------
+#pragma unroll
+  for (int r = 0; r < E; ++r) X[r] = kzb[(f * NZ + j + T * r) * TYL + line];
+  fft_stage1<E, true>(X, w);
+#pragma unroll
+  for (int q = 0; q < E; ++q) buf[q * QS + j * TYL + line] = X[q];
+  __syncthreads();
+  fft_stage2<E, T, true>(X, j, [&](int q, int jj) { return buf[q * QS + jj * TYL + line]; });
+  {
+    float2* __restrict__ out = (f == 0 ? (emit ? g.e0 : g.v0) : (emit ? g.e1 : g.v1)) + slab;
+#pragma unroll
+    for (int r = 0; r < E; ++r) out[(size_t)(j + T * r) * y2] = X[r];
   }
 }
 

@@ -15,8 +15,10 @@ namespace wt {
 // ------------------------------------------------------------------------------------------------
 template <bool APPLY_J, bool DELTA>
 __global__ void __launch_bounds__(256) k_spectral(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emit) {
+  pdl_trigger();
   const GeomDev& g = gb.g[blockIdx.y];
-  if (substep >= g.n_sub) return;
+  if (substep >= g.n_sub) { pdl_wait(); return; }
+  pdl_wait();
   const int nx = gd.nx, nz = gd.nz, y2 = gd.y2, TY = gd.ty;
   const int tiles = y2 / TY;
   const int kx = blockIdx.x / tiles, ky0 = (blockIdx.x % tiles) * TY;
@@ -126,8 +128,10 @@ __global__ void __launch_bounds__(256) k_spectral(const __grid_constant__ GeomBa
 // ------------------------------------------------------------------------------------------------
 template <bool EMIT>
 __global__ void __launch_bounds__(256) k_plane(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
+  pdl_trigger();
   const GeomDev& g = gb.g[blockIdx.y];
-  if (substep >= g.n_sub) return;
+  if (substep >= g.n_sub) { pdl_wait(); return; }
+  pdl_wait();
   const int nx = gd.nx, ny = gd.ny, nz = gd.nz, y2 = gd.y2;
   const int z = blockIdx.x;
   const int tid = threadIdx.x, bd = blockDim.x;
@@ -242,6 +246,8 @@ __global__ void __launch_bounds__(256) k_plane(const __grid_constant__ GeomBatch
 // ------------------------------------------------------------------------------------------------
 template <bool YX>
 __global__ void __launch_bounds__(256) k_transpose(const __grid_constant__ GeomBatch gb, GridDev gd) {
+  pdl_trigger();
+  pdl_wait();
   const int n = *gd.step;
   if (!((n + 1) % kStageSlots == 0 || n == gd.nt - 1)) return;
   const int cnt = n % kStageSlots + 1, t0 = n - cnt + 1;
@@ -264,6 +270,10 @@ __global__ void __launch_bounds__(256) k_transpose(const __grid_constant__ GeomB
   }
 }
 
-__global__ void k_advance(int* step) { *step += 1; }
+__global__ void k_advance(int* step) {
+  pdl_trigger();
+  pdl_wait();
+  *step += 1;
+}
 
 }  // namespace wt
