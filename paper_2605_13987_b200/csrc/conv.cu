@@ -2,12 +2,18 @@
 //
 // PAPER.md:35-39 (Eq. 1.1), :74 ("for each charge carrier, the induced signal is computed as
 // described in Equation 1.1"), :99 (one carrier per CUDA thread, H through texture interpolation).
-// Here: one CTA per carrier, threads own output times n, the 8 corner rows of the time-innermost
-// table are read with coalesced loads (consecutive threads = consecutive lags), trilinear weights
-// in full fp32 (R23).  Per-track sums are formed in a second pass in carrier order (R25).
+// Two kernels compute the same sums:
+//   k_conv_systolic (nt <= 1024)  one CTA per group of consecutive carriers; lanes own FLOATS of the
+//       time-innermost rows (16-byte aligned, fully coalesced 128-bit loads) and the partial sums
+//       travel across the lanes by warp shuffles as the step index advances (see the kernel);
+//   k_conv_carrier (any nt)       one CTA per carrier, threads own output times n.
+// Trilinear weights in full fp32 (R23).  Per-track sums are formed in carrier order from partial
+// rows in a second pass (R25: fixed order, no float atomics).
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cstdint>
+#include <cstdlib>
 #include <string>
 
 #include "geometry.h"
@@ -121,14 +127,200 @@ __global__ void __launch_bounds__(kThreads) k_conv_carrier(ConvParams p) {
   }
 }
 
-// a12: i_track[n] = sum over the track's carriers in carrier order (fixed order: deterministic)
+// ------------------------------------------------------------------------------------------------
+// k_conv_systolic: Eq. 1.1 with the table rows read where they lie.
+//
+// A node row is F = 3 nt floats, float f = 3 lag + component.  Step m, corner k adds
+//   c[m][k][f % 3] * row_k[f]   to the partial sum   S[f + 3 m],       i(n) = S[3n] + S[3n+1] + S[3n+2].
+// Warp w owns the floats [384 w, 384 w + 384) of every row: lane t holds f = 384 w + 128 j + 4 t + i
+// (j < 3, i < 4), i.e. three 128-bit loads per corner that are 16-byte aligned for every step and
+// cover 512 contiguous bytes per instruction.  The twelve partial sums of a lane belong to S[f + 3 m]:
+// when m advances they move down by three floats, i.e. one register rotation plus three shuffles per
+// 128-float group; sums that leave the warp's range at the bottom are complete (for this warp) and go
+// to the warp's own row P_w in shared memory, each element written once per carrier, so the result
+// does not depend on scheduling (R25).  Component of (j, i) = (t + 2 j + i) % 3: the three weights of
+// a corner are rotated by t % 3 once per corner with selects.
+// One CTA handles `gc` consecutive carriers; with per_track the rows of carriers of one track are
+// summed in P (carrier order) and written as one partial row at the index of the segment's first carrier.
+// grid = ceil(n_carriers / gc), block = 32 * ceil(nt / 128) <= 256,
+// dynamic smem = kStepChunk * 8 * 16 + nw * 3 nt * 4 bytes.
+// ------------------------------------------------------------------------------------------------
+constexpr int kStepChunk = 32;
+
+struct SysParams {
+  ConvParams c;
+  const int64_t* track_off;   // [n_tracks + 1] (per_track) or NULL
+  int64_t n_tracks, n_carriers;
+  int gc, stride, per_track;   // a CTA handles carriers base + s, base + s + stride, ... (gc of them)
+};
+
+__device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+
+__global__ void __launch_bounds__(256, 2) k_conv_systolic(SysParams sp) {
+  const ConvParams& p = sp.c;
+  const int nt = p.nt, F = 3 * nt;
+  const int tid = threadIdx.x, w = tid >> 5, t = tid & 31, nw = blockDim.x >> 5;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  float4* tab = reinterpret_cast<float4*>(smraw);                                // [kStepChunk][8]  (node bits, c0, c1, c2)
+  float* P = reinterpret_cast<float*>(smraw + kStepChunk * 8 * sizeof(float4));   // [nw][F]
+  float* Pw = P + (size_t)w * F;
+  __shared__ int64_t s_track;
+
+  const int f0 = 384 * w + 4 * t;
+  const bool v0 = f0 < F, v1 = f0 + 128 < F, v2 = f0 + 256 < F;       // F % 4 == 0: whole 16-byte groups
+  const int r = t % 3;
+  const bool r0 = (r == 0), r1 = (r == 1);
+
+  // carriers of this CTA: cb, cb + S, cb + 2 S, ... (gc of them, inside one super-group of gc * S carriers):
+  // the S CTAs of a super-group work on S adjacent carriers at any time, whose rows largely coincide (L2 reuse)
+  const int S = sp.stride;
+  const int64_t sgb = (int64_t)(blockIdx.x / S) * sp.gc * S;
+  const int64_t cb = sgb + blockIdx.x % S, ce = min(sp.n_carriers, sgb + (int64_t)sp.gc * S);
+  if (cb >= ce) return;
+  // track of the first carrier: largest tr with track_off[tr] <= cb
+  int64_t tr = 0, c_next = 0x7fffffffffffffffLL, seg = cb;
+  if (sp.per_track) {
+    if (tid == 0) {
+      int64_t lo = 0, hi = sp.n_tracks;            // invariant: track_off[lo] <= cb (track_off[0] may exceed cb: handled below)
+      while (lo < hi) { const int64_t mid = (lo + hi + 1) >> 1; if (sp.track_off[mid] <= cb) lo = mid; else hi = mid - 1; }
+      s_track = lo;
+    }
+    __syncthreads();
+    tr = s_track;
+    if (tr >= sp.n_tracks) return;                 // carriers past the last track belong to no row
+    c_next = sp.track_off[tr + 1];
+    seg = max(cb, sp.track_off[tr]);               // first carrier index that can open a segment
+  }
+  for (int i = tid; i < nw * F; i += blockDim.x) P[i] = 0.f;
+  __syncthreads();
+  bool opened = false;
+
+  // writes i(n) = sum_w S_w[3n..3n+2] to the output row and clears P
+  auto flush_row = [&](float* __restrict__ row) {
+    __syncthreads();
+    for (int n = tid; n < nt; n += blockDim.x) {
+      float s = 0.f;
+      for (int ww = 0; ww < nw; ++ww) {
+        const float* q = P + (size_t)ww * F + 3 * n;
+        s += (q[0] + q[1]) + q[2];
+      }
+      row[n] = s;
+    }
+    __syncthreads();
+    for (int i = tid; i < nw * F; i += blockDim.x) P[i] = 0.f;
+    __syncthreads();
+  };
+
+  for (int64_t c = cb; c < ce; c += S) {
+    if (c < seg) continue;                         // (carriers before the first track belong to no row)
+    if (sp.per_track && c >= c_next) {             // the track changes inside the group
+      if (opened) flush_row(p.out + (size_t)seg * nt);
+      opened = false;
+      while (tr < sp.n_tracks && c >= sp.track_off[tr + 1]) ++tr;
+      if (tr >= sp.n_tracks) return;
+      c_next = sp.track_off[tr + 1];
+    }
+    if (!opened) { opened = true; seg = c; }       // partial rows live at the index of the segment's first carrier
+    const int64_t s0 = p.carrier_off[c];
+    const int M = (int)min((int64_t)nt, p.carrier_off[c + 1] - s0);   // steps m >= nt are ignored (R26)
+    const float scale = -p.charge[c] * p.dt_over_vw;
+    float A[3][4];
+#pragma unroll
+    for (int j = 0; j < 3; ++j)
+#pragma unroll
+      for (int i = 0; i < 4; ++i) A[j][i] = 0.f;
+
+    // m -> m + 1: the sums move down by three floats; the three lowest of the warp are complete
+    auto shift = [&](int m) {
+      if (t == 0) {
+        const int gq = 384 * w + 3 * m;
+        if (gq < F) { Pw[gq] += A[0][0]; Pw[gq + 1] += A[0][1]; Pw[gq + 2] += A[0][2]; }   // F % 3 == 0
+      }
+      float sh[3][3];
+#pragma unroll
+      for (int j = 0; j < 3; ++j)
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+          const float up = (j < 2) ? A[j + 1][i] : 0.f;
+          sh[j][i] = __shfl_sync(0xffffffffu, t == 0 ? up : A[j][i], (t + 1) & 31);
+        }
+#pragma unroll
+      for (int j = 0; j < 3; ++j) { A[j][0] = A[j][3]; A[j][1] = sh[j][0]; A[j][2] = sh[j][1]; A[j][3] = sh[j][2]; }
+    };
+    // one (step, corner) entry e = (., c_x, c_y, c_z) applied to the lane's twelve floats of the corner's row
+    auto fma12 = [&](float (&D)[3][4], const float4 e, const float4 h0, const float4 h1, const float4 h2) {
+      const float q0 = r0 ? e.y : (r1 ? e.z : e.w);      // weight of component (t + x) % 3, x = 0, 1, 2
+      const float q1 = r0 ? e.z : (r1 ? e.w : e.y);
+      const float q2 = r0 ? e.w : (r1 ? e.y : e.z);
+      D[0][0] = fmaf(q0, h0.x, D[0][0]); D[0][1] = fmaf(q1, h0.y, D[0][1]); D[0][2] = fmaf(q2, h0.z, D[0][2]); D[0][3] = fmaf(q0, h0.w, D[0][3]);
+      D[1][0] = fmaf(q2, h1.x, D[1][0]); D[1][1] = fmaf(q0, h1.y, D[1][1]); D[1][2] = fmaf(q1, h1.z, D[1][2]); D[1][3] = fmaf(q2, h1.w, D[1][3]);
+      D[2][0] = fmaf(q1, h2.x, D[2][0]); D[2][1] = fmaf(q2, h2.y, D[2][1]); D[2][2] = fmaf(q0, h2.z, D[2][2]); D[2][3] = fmaf(q1, h2.w, D[2][3]);
+    };
+    const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+
+    {
+      for (int m0 = 0; m0 < M; m0 += kStepChunk) {
+        const int mc = min(kStepChunk, M - m0);
+        __syncthreads();
+        if (tid < mc) {
+          const int64_t s = s0 + m0 + tid;
+          const float vx = p.vel[3 * s], vy = p.vel[3 * s + 1], vz = p.vel[3 * s + 2];
+          const NodeFrac nf = locate(p.pos[3 * s], p.pos[3 * s + 1], p.pos[3 * s + 2], p.nx, p.ny, p.nz, p.invx, p.invy, p.invz);
+          const bool ok = nf.ok && isfinite(vx) && isfinite(vy) && isfinite(vz);
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const int cx = k >> 2, cy = (k >> 1) & 1, cz = k & 1;
+            const float wgt = (cx ? nf.f[0] : 1.f - nf.f[0]) * (cy ? nf.f[1] : 1.f - nf.f[1]) * (cz ? nf.f[2] : 1.f - nf.f[2]);
+            const int ix = cx ? nf.i1[0] : nf.i0[0], iy = cy ? nf.i1[1] : nf.i0[1], iz = cz ? nf.i1[2] : nf.i0[2];
+            const unsigned node = ok ? (unsigned)((ix * p.ny + iy) * p.nz + iz) : 0u;
+            const float ws = wgt * scale;            // a non-finite step contributes nothing (0, not 0 * inf)
+            tab[tid * 8 + k] = make_float4(__uint_as_float(node), ok ? ws * vx : 0.f, ok ? ws * vy : 0.f, ok ? ws * vz : 0.f);
+          }
+        }
+        __syncthreads();
+        for (int jm = 0; jm < mc; ++jm) {
+          const int m = m0 + jm;
+          if (128 * w + m >= nt) break;              // every output of this warp is past nt from here on (warp uniform)
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {
+            const float4 e = tab[jm * 8 + k];
+            const float* __restrict__ src = p.H + (size_t)__float_as_uint(e.x) * F + f0;
+            const float4 h0 = v0 ? ldg4(src) : z4, h1 = v1 ? ldg4(src + 128) : z4, h2 = v2 ? ldg4(src + 256) : z4;
+            fma12(A, e, h0, h1, h2);
+          }
+          shift(m);
+        }
+      }
+    }
+    // after M steps lane (j, i) holds S[f + 3 M]
+    __syncwarp();
+#pragma unroll
+    for (int j = 0; j < 3; ++j)
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        const int gq = f0 + 128 * j + i + 3 * M;
+        if (f0 + 128 * j < F && gq < F) Pw[gq] += A[j][i];   // (a warp that left the loop early holds outputs >= nt only)
+      }
+    __syncwarp();
+    if (!sp.per_track) flush_row(p.out + (size_t)c * nt);
+  }
+  if (sp.per_track && opened) flush_row(p.out + (size_t)seg * nt);
+}
+
+// a12: i_track[n] = sum of the partial rows of the track in carrier order (fixed order: deterministic).
+// A CTA of the convolution kernel handles the carriers base + s + i * stride (i < gc) of a super-group of
+// gc * stride carriers and leaves one partial row per track segment at the index of the segment's first
+// carrier; gc = 1: one row per carrier.
 __global__ void __launch_bounds__(256) k_track_sum(const float* __restrict__ cur, const int64_t* __restrict__ track_off,
-                                                   float* __restrict__ out, int nt) {
+                                                   float* __restrict__ out, int nt, int gc, int stride) {
   const int64_t t = blockIdx.x;
-  const int64_t c0 = track_off[t], c1 = track_off[t + 1];
+  const int64_t c0 = track_off[t], c1 = track_off[t + 1], sg = (int64_t)gc * stride;
   for (int n = threadIdx.x; n < nt; n += blockDim.x) {
     float s = 0.f;
-    for (int64_t c = c0; c < c1; ++c) s += cur[(size_t)c * nt + n];
+    for (int64_t c = c0; c < c1; ++c) {
+      const int64_t prev = c - stride;             // the carrier the same CTA handled before c
+      if (prev < c0 || prev < c / sg * sg) s += cur[(size_t)c * nt + n];   // c opened a segment
+    }
     out[(size_t)t * nt + n] = s;
   }
 }
@@ -142,6 +334,11 @@ __global__ void k_nodes(int64_t n_steps, const float* __restrict__ pos, int32_t*
 }
 
 inline size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+bool env_flag(const char* name) {
+  const char* v = std::getenv(name);
+  return v && v[0] && v[0] != '0';
+}
 
 }  // namespace
 
@@ -177,11 +374,30 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
   p.nx = g->nx; p.ny = g->ny; p.nz = g->nz; p.nt = g->nt;
   p.invx = (float)((double)g->nx / g->lx); p.invy = (float)((double)g->ny / g->ly); p.invz = (float)((double)g->nz / g->lz);
   p.dt_over_vw = (float)(g->dt / g->v_w);
-  if (n_carriers > 0) ++g_wt_launches;
-  if (n_carriers > 0) k_conv_carrier<<<(unsigned)n_carriers, kThreads, 0, st>>>(p);
-  if (per_track && n_tracks > 0) ++g_wt_launches;
-  if (per_track && n_tracks > 0)
-    k_track_sum<<<(unsigned)n_tracks, 256, 0, st>>>((const float*)workspace_dev, track_carrier_offsets_dev, out_dev, g->nt);
+  // kernel choice: the systolic kernel for nt <= 1024 (its per-warp rows fit in shared memory), else one CTA per carrier
+  static const bool force_v1 = env_flag("WTIDE_CONV_V1");
+  const int nw = (g->nt + 127) / 128;
+  int gc = 1, stride = 1;
+  if (n_carriers > 0 && nw <= 8 && !force_v1) {
+    if (per_track && n_carriers >= 148 * 8 * 8) { gc = 8; stride = 32; }   // carriers per CTA: amortises the row combine
+    SysParams sp;
+    sp.c = p; sp.track_off = per_track ? track_carrier_offsets_dev : nullptr;
+    sp.n_tracks = n_tracks; sp.n_carriers = n_carriers; sp.gc = gc; sp.stride = stride; sp.per_track = per_track ? 1 : 0;
+    const size_t smem = (size_t)kStepChunk * 8 * sizeof(float4) + (size_t)nw * 3 * g->nt * sizeof(float);
+    auto fn = k_conv_systolic;
+    cudaError_t ea = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (ea != cudaSuccess) { wt_set_error(std::string("wt_convolve_currents: ") + cudaGetErrorString(ea)); return WT_ECUDA; }
+    ++g_wt_launches;
+    const int64_t sg = (int64_t)gc * stride;
+    fn<<<(unsigned)((n_carriers + sg - 1) / sg * stride), 32 * nw, smem, st>>>(sp);
+  } else if (n_carriers > 0) {
+    ++g_wt_launches;
+    k_conv_carrier<<<(unsigned)n_carriers, kThreads, 0, st>>>(p);
+  }
+  if (per_track && n_tracks > 0) {
+    ++g_wt_launches;
+    k_track_sum<<<(unsigned)n_tracks, 256, 0, st>>>((const float*)workspace_dev, track_carrier_offsets_dev, out_dev, g->nt, gc, stride);
+  }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { wt_set_error(std::string("wt_convolve_currents: ") + cudaGetErrorString(e)); return WT_ECUDA; }
   wt_set_error("");

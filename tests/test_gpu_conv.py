@@ -145,3 +145,38 @@ def test_full_size_table_sampled_tracks():
     ref = _oracle(d, rows, csr, True)
     l2, mx = wo.current_error(got, ref)
     assert l2 <= TOL and mx <= 5 * TOL, (l2, mx)
+
+
+def test_many_carriers_ragged_tracks_grouped_path():
+    """Enough carriers for the grouped launch (8 carriers per CTA, interleaved over 32 CTAs, partial rows
+    per track segment): ragged tracks incl. empty ones, carriers before the first and after the last
+    track, empty carriers; per-track and per-carrier outputs against the oracle."""
+    nt = 20
+    d = reduced_desc(geometry_desc(0), grid=(8, 8, 6), nt=nt)
+    g = wt.wt_make_geometry(d)
+    rng = np.random.default_rng(7)
+    Hnp = rng.standard_normal((8, 8, 6, nt, 3)).astype(np.float32)
+    H = torch.as_tensor(Hnp).to(DEV)
+    n_car = 12_000
+    lens = rng.integers(0, 5, size=n_car)
+    lens[100] = nt + 3
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    S = int(off[-1])
+    pos = rng.uniform(-20, 70, size=(S, 3)).astype(np.float32)
+    vel = rng.standard_normal((S, 3)).astype(np.float32)
+    # tracks: a few carriers before the first track and after the last belong to no track
+    cuts = np.sort(rng.choice(np.arange(5, n_car - 5), size=60, replace=False))
+    toff = np.concatenate([[3], cuts, cuts[10:13], [n_car - 4]]).astype(np.int64)   # repeated cuts = empty tracks
+    toff.sort()
+    csr = dict(track_carrier_offsets=toff, carrier_step_offsets=off, pos=pos, vel=vel,
+               charge=rng.standard_normal(n_car).astype(np.float32))
+    ref_c = _oracle(d, Hnp, csr, False)
+    got_c = _run(g, H, csr, False)
+    scale = np.abs(ref_c).max()
+    assert np.abs(got_c - ref_c).max() <= TOL * scale
+    got_t = _run(g, H, csr, True)
+    ref_t = np.stack([ref_c[toff[i]:toff[i + 1]].sum(axis=0) for i in range(len(toff) - 1)])
+    assert got_t.shape == ref_t.shape
+    assert np.abs(got_t - ref_t).max() <= TOL * np.abs(ref_t).max()
+    empty = np.nonzero(np.diff(toff) == 0)[0]
+    assert len(empty) >= 3 and (got_t[empty] == 0).all()
