@@ -315,13 +315,36 @@ __global__ void __launch_bounds__(256) k_track_sum(const float* __restrict__ cur
                                                    float* __restrict__ out, int nt, int gc, int stride) {
   const int64_t t = blockIdx.x;
   const int64_t c0 = track_off[t], c1 = track_off[t + 1], sg = (int64_t)gc * stride;
-  for (int n = threadIdx.x; n < nt; n += blockDim.x) {
-    float s = 0.f;
-    for (int64_t c = c0; c < c1; ++c) {
-      const int64_t prev = c - stride;             // the carrier the same CTA handled before c
-      if (prev < c0 || prev < c / sg * sg) s += cur[(size_t)c * nt + n];   // c opened a segment
+  __shared__ int64_t rows[256];
+  __shared__ int n_rows;
+  __shared__ int64_t c_resume;
+  for (int nb = 0; nb < nt; nb += 4 * 256) {
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+    int64_t c = c0;
+    while (c < c1) {                                 // (uniform: c comes from shared memory)
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        // segment starts: carriers whose predecessor in their CTA (c - stride) lies outside the track or the super-group
+        int k = 0;
+        while (c < c1 && k < 256) {
+          const int64_t base = c / sg * sg;
+          if (c - stride < c0 || c - stride < base) rows[k++] = c++;
+          else c = base + sg;
+        }
+        n_rows = k; c_resume = c;
+      }
+      __syncthreads();
+      for (int r = 0; r < n_rows; ++r) {
+        const float* __restrict__ row = cur + (size_t)rows[r] * nt + nb + threadIdx.x;
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+          if (nb + i * 256 + (int)threadIdx.x < nt) acc[i] += row[i * 256];
+      }
+      c = c_resume;
     }
-    out[(size_t)t * nt + n] = s;
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+      if (nb + i * 256 + (int)threadIdx.x < nt) out[(size_t)t * nt + nb + i * 256 + threadIdx.x] = acc[i];
   }
 }
 
