@@ -340,15 +340,23 @@ def run_ours(args):
         conv_gbs = alg_conv_bytes / (conv_ms * 1e-3) / 1e9
         solve_gbs = alg_solve_bytes / (solve_ms * 1e-3) / 1e9
         dominant_is_solve = solve_ms >= conv_ms
+        # DRAM bytes from the ncu --set full captures of this workload (profiles/r1_solve.md, profiles/r1_conv.md):
+        # solve = 35.9 MB per substep in the cold-cache capture of its three kernels (an upper bound: in the replayed
+        # graph the working set is L2-resident); Eq. 1.1 = 154.4 GB per call at 1000 tracks x 1000 carriers.
+        default_workload = (args.tracks == 1000 and args.carriers == 1000 and not args.grid and not args.nt)
+        traffic_solve = 35.9e6 * n_sub * (nt - 1) if default_workload else None
+        traffic_conv = 154.4e9 if default_workload else None
         roof = {"bound": "hbm", "kernel": "wt_solve_H (k_plane + k_spectral + boundary kernels, all substeps)" if dominant_is_solve
                 else "k_conv_systolic", "achieved": solve_gbs if dominant_is_solve else conv_gbs, "peak": peak, "unit": "GB/s",
-                "frac": (solve_gbs if dominant_is_solve else conv_gbs) / peak, "traffic": None, "peak_source": peak_kind,
+                "frac": (solve_gbs if dominant_is_solve else conv_gbs) / peak,
+                "traffic": traffic_solve if dominant_is_solve else traffic_conv, "peak_source": peak_kind,
                 "algorithmic_bytes": alg_solve_bytes if dominant_is_solve else alg_conv_bytes}
         stages = {"solve_ms": solve_ms, "conv_ms": conv_ms,
                   "solve": {"algorithmic_bytes": alg_solve_bytes, "achieved_gbs": solve_gbs, "frac": solve_gbs / peak,
+                            "traffic": traffic_solve,
                             "n_sub": n_sub, "substeps": n_sub * (nt - 1), "us_per_substep": 1e3 * solve_ms / (n_sub * (nt - 1)), "pads": n_pads},
                   "conv": {"algorithmic_bytes": alg_conv_bytes, "no_reuse_gather_bytes": 96 * terms, "achieved_gbs": conv_gbs,
-                           "frac": conv_gbs / peak, "carriers": n_car, "carrier_steps": n_steps_total,
+                           "frac": conv_gbs / peak, "traffic": traffic_conv, "carriers": n_car, "carrier_steps": n_steps_total,
                            "mean_steps": n_steps_total / max(1, n_car)}}
         line = {"metric": METRIC, "value": total_terms / (conv_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
