@@ -51,6 +51,13 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
 
   float2 w[E];
   load_twiddles<E>(w, g.twx, j);          // N x N plane: twx == twy
+  // small tables that are needed in the middle and at the end of the kernel go to shared memory now, while the
+  // predecessor is still running: a global load there would stall every warp of the CTA with nothing to overlap
+  __shared__ float s_sdt[256];
+  __shared__ float s_kx[N];
+  if (!EMIT)
+    for (int i = tid; i < 256; i += N * N / (2 * E)) s_sdt[i] = __ldg(g.sdt + i);
+  for (int i = tid; i < N; i += N * N / (2 * E)) s_kx[i] = __ldg(g.kxf + i);
 
   // conductivity ids of this thread's nodes in the y-phases: rows 2 ln, 2 ln + 1 at y = j + T r
   unsigned short sid[E];
@@ -60,13 +67,14 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
     for (int r = 0; r < E; ++r) sid[r] = __ldg(st + ((j + T * r) * N + 2 * ln) / 2);
   }
 
+  const float kyv = __ldg(g.kyf + ln);
+  __syncthreads();
   pdl_wait();
   float2 X[E];
   // ---- load: V~ = V~_rho + sum_l Q^_l g~(z - z_l) (the boundary source, a4); E~ = -i kappa V~ ------------
   {
     const float2* __restrict__ src = EMIT ? (comp == 2 ? g.e1 : g.e0) : (comp == 2 ? g.v1 : g.v0);
     const float* __restrict__ tab = (comp == 2) ? g.gzt : g.gt;
-    const float kyv = g.kyf[ln];
 #pragma unroll
     for (int r = 0; r < E; ++r) {
       const int kx = j + T * r;
@@ -88,7 +96,7 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
     if (comp < 2) {
 #pragma unroll
       for (int r = 0; r < E; ++r) {
-        const float kap = (comp == 0) ? g.kxf[j + T * r] : kyv;
+        const float kap = (comp == 0) ? s_kx[j + T * r] : kyv;
         X[r] = make_float2(kap * X[r].y, -kap * X[r].x);       // -i kappa V~
       }
     }
@@ -136,8 +144,8 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
   // ---- conduction current J = (s dt_int) E, nodewise (a6, R17) ----------------------------------------------
 #pragma unroll
   for (int r = 0; r < E; ++r) {
-    X[r].x *= __ldg(g.sdt + (sid[r] & 0xff));
-    X[r].y *= __ldg(g.sdt + (sid[r] >> 8));
+    X[r].x *= s_sdt[sid[r] & 0xff];
+    X[r].y *= s_sdt[sid[r] >> 8];
   }
   // ---- C: forward transform along y ---------------------------------------------------------------------
   fft_stage1<E, false>(X, w);
@@ -169,13 +177,12 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
   // ---- out: i kx J~x | i ky J~y | J~z ----------------------------------------------------------------------
   {
     float2* __restrict__ dst = (comp == 0) ? g.m0 : (comp == 1) ? g.m1 : g.m2;
-    const float kyv = g.kyf[ln];
 #pragma unroll
     for (int r = 0; r < E; ++r) {
       const int kx = j + T * r;
       float2 o = X[r];
       if (comp < 2) {
-        const float kap = (comp == 0) ? g.kxf[kx] : kyv;
+        const float kap = (comp == 0) ? s_kx[kx] : kyv;
         o = make_float2(-kap * o.y, kap * o.x);
       }
       dst[((size_t)kx * nz + z) * Y2 + ln] = o;
@@ -369,6 +376,13 @@ k_pencil2(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emi
   float2 w[E];
   load_twiddles<E>(w, g.twz, j);
   float2 X[E];
+  // wavenumbers and fp64 twiddles of the per-mode update: to shared memory during the prologue (a global
+  // load in the middle of the kernel stalls all warps of the CTA with nothing to overlap)
+  __shared__ double s_kz[NZ];
+  __shared__ double2 s_twz[NZ];
+  for (int i = tid; i < NZ; i += 2 * HT) { s_kz[i] = g.kzd[i]; s_twz[i] = g.twzd[i]; }
+  const double kxd = g.kxd[kx], kyd = g.kyd[ky];
+  __syncthreads();
   pdl_wait();
 
   if constexpr (APPLY_J) {
@@ -403,7 +417,6 @@ k_pencil2(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emi
     double2 acc[LT];
 #pragma unroll
     for (int l = 0; l < LT; ++l) acc[l] = make_double2(0.0, 0.0);
-    const double kxd = g.kxd[kx], kyd = g.kyd[ky];
     const double kxy2 = kxd * kxd + kyd * kyd;
     const bool ret_x = (kx != nx / 2);
     double2* __restrict__ rh = g.rhat + slab;
@@ -413,7 +426,7 @@ k_pencil2(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emi
       const int kz = j + T * (2 * i + f);
       const size_t o = (size_t)kz * y2;
       const bool ret = ret_x && (kz != NZ / 2);
-      const double kzd = g.kzd[kz];
+      const double kzd = s_kz[kz];
       double2 rr = rh[o];
       if constexpr (APPLY_J) {
         const float2 D = kzb[kz * TYL + line], J = kzb[(NZ + kz) * TYL + line];
@@ -437,7 +450,7 @@ k_pencil2(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emi
 #pragma unroll
       for (int l = 0; l < LT; ++l) {
         if (l < L) {
-          double2 ww = g.twzd[(kz * g.layers[l]) & (NZ - 1)];
+          double2 ww = s_twz[(kz * g.layers[l]) & (NZ - 1)];
           ww.y = -ww.y;                                                 // e^{+i kz z_l}
           const double2 p = dmul(v, ww);
           acc[l].x += p.x; acc[l].y += p.y;

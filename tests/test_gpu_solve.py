@@ -123,3 +123,21 @@ def test_cfg1_window_matches_the_oracle_at_sampled_rows():
     _, (h,) = _solve([d])
     ref = wo.solve_H_from_desc(d)
     assert wo.h_rel_l2(h, ref) <= TOL
+
+
+def test_every_config_geometry_on_a_reduced_grid():
+    """The geometries of BASELINE.json configs 2, 3 and 4 (hexagonal stand-in with 7 columns; two cells of the
+    what-if sweep solved in lock step; the radix-3 grid of the high-statistics config) on grids the oracle
+    finishes in seconds, 3 output steps each, n_sub as the geometry demands."""
+    from wtide_inputs.configs import sweep_descs
+    d2 = reduced_desc(geometry_desc(2), grid=(32, 32, 16), nt=4)
+    d4 = reduced_desc(geometry_desc(4), grid=(24, 24, 48), nt=4)
+    sw = sweep_descs(grid=(16, 16, 32), nt=4)
+    d3a, d3b = sw[10], sw[11]                    # pitch 55 um, bias radius 5 um, resistivity 0.1 and 1 ohm cm
+    for d in (d2, d4):
+        _, (h,) = _solve([d])
+        assert wo.h_rel_l2(h, wo.solve_H_from_desc(d)) <= TOL
+    geoms, (ha, hb) = _solve([d3a, d3b])
+    assert wt.wt_query(geoms[0], wt.WT_Q_SUBSTEPS) == 10 * wt.wt_query(geoms[1], wt.WT_Q_SUBSTEPS)
+    for h, d in ((ha, d3a), (hb, d3b)):
+        assert wo.h_rel_l2(h, wo.solve_H_from_desc(d)) <= TOL
