@@ -187,6 +187,27 @@ def run_reference(args):
 
 
 # --------------------------------------------------------------------------------------------------
+# multi-GPU: replicas only.  Tracks are the independent units: rank r
+# takes tracks [r * n, (r + 1) * n) of the seeded track list; the only collectives are the timing ones.
+# --------------------------------------------------------------------------------------------------
+def shard_tracks(tracks_per_rank, world, rank):
+    assert 0 <= rank < world
+    return slice(rank * tracks_per_rank, (rank + 1) * tracks_per_rank)
+
+
+def reduce_over_ranks(times_ms, work, world, device):
+    """MAX of the per-rank times, SUM of the per-rank work (terms); identity for world == 1."""
+    import torch
+    vals = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    tot = torch.tensor([float(work)], dtype=torch.float64, device=device)
+    if world > 1:
+        import torch.distributed as dist
+        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    return [float(v) for v in vals.cpu()], float(tot.cpu()[0])
+
+
+# --------------------------------------------------------------------------------------------------
 # our arm
 # --------------------------------------------------------------------------------------------------
 def unique_row_bytes(wt, g, csr_dev, nt, n_nodes, chunk_carriers=50_000):
@@ -255,7 +276,7 @@ def run_ours(args):
     wt.wt_solve_H([g], H=H, workspace=ws_solve, device=dev)
     torch.cuda.synchronize()
     e_static = H[0].view(n_nodes, nt, 3).sum(dim=1).mul_(d["dt"]).view(d["nx"], d["ny"], d["nz"], 3)
-    tracks = make_tracks(1, args.tracks * world, d, 10.0)[rank * args.tracks:(rank + 1) * args.tracks]
+    tracks = make_tracks(1, args.tracks * world, d, 10.0)[shard_tracks(args.tracks, world, rank)]
     start, sign, charge, toff = carriers_on_tracks(tracks, args.carriers, d)
     csr = field_drift(e_static, d, start, sign, charge, toff)
     del e_static
@@ -321,13 +342,7 @@ def run_ours(args):
     e2e_s = (time.perf_counter() - t0) / args.steps
 
     # ---- reduce over ranks (max time, summed work)
-    vals = torch.tensor([solve_ms, conv_ms, step_ms, e2e_s * 1e3], dtype=torch.float64, device=dev)
-    work = torch.tensor([float(terms)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
-        dist.all_reduce(work, op=dist.ReduceOp.SUM)
-    solve_ms, conv_ms, step_ms, e2e_ms = (float(v) for v in vals.cpu())
-    total_terms = float(work.cpu()[0])
+    (solve_ms, conv_ms, step_ms, e2e_ms), total_terms = reduce_over_ranks([solve_ms, conv_ms, step_ms, e2e_s * 1e3], terms, world, dev)
 
     if rank == 0:
         peak, peak_kind = measured_peaks()
