@@ -40,7 +40,7 @@ def measured_peaks():
 
 def workload(args):
     from wtide_inputs import geometry_desc, reduced_desc
-    d = geometry_desc(1, seed=0)
+    d = geometry_desc(args.config, seed=0)
     if args.grid:
         nx, ny, nz = (int(v) for v in args.grid.split("x"))
         d = reduced_desc(d, grid=(nx, ny, nz))
@@ -276,7 +276,8 @@ def run_ours(args):
     wt.wt_solve_H([g], H=H, workspace=ws_solve, device=dev)
     torch.cuda.synchronize()
     e_static = H[0].view(n_nodes, nt, 3).sum(dim=1).mul_(d["dt"]).view(d["nx"], d["ny"], d["nz"], 3)
-    tracks = make_tracks(1, args.tracks * world, d, 10.0)[shard_tracks(args.tracks, world, rank)]
+    theta_max = 15.0 if args.config == 4 else 10.0
+    tracks = make_tracks(args.config, args.tracks * world, d, theta_max)[shard_tracks(args.tracks, world, rank)]
     start, sign, charge, toff = carriers_on_tracks(tracks, args.carriers, d)
     csr = field_drift(e_static, d, start, sign, charge, toff)
     del e_static
@@ -388,7 +389,7 @@ def run_ours(args):
         # DRAM bytes from the ncu --set full captures of this workload (profiles/r1_solve.md, profiles/r1_conv.md):
         # solve = 35.9 MB per substep in the cold-cache capture of its three kernels (an upper bound: in the replayed
         # graph the working set is L2-resident); Eq. 1.1 = 154.4 GB per call at 1000 tracks x 1000 carriers.
-        default_workload = (args.tracks == 1000 and args.carriers == 1000 and not args.grid and not args.nt)
+        default_workload = (args.config == 1 and args.tracks == 1000 and args.carriers == 1000 and not args.grid and not args.nt)
         traffic_solve = 35.9e6 * n_sub * (nt - 1) if default_workload else None
         traffic_conv = 154.4e9 if default_workload else None
         roof = {"bound": "hbm", "kernel": "wt_solve_H (k_plane_fast + k_pencil2 + k_boundary_fast, all substeps)" if dominant_is_solve
@@ -406,8 +407,10 @@ def run_ours(args):
         line = {"metric": METRIC, "value": total_terms / (conv_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
-                "config": {"workload": "configs[1] single pixel cell 55um x 500um, grid %dx%dx%d, nt=%d, dt=%g ns, %d tracks x %d carriers per GPU"
-                           % (d["nx"], d["ny"], d["nz"], nt, d["dt"], args.tracks, args.carriers),
+                "config": {"workload": "configs[%d] %s, grid %dx%dx%d, nt=%d, dt=%g ns, %d tracks x %d carriers per GPU"
+                           % (args.config, {1: "single pixel cell 55um x 500um", 2: "hexagonal stand-in 128um x 500um, 7 columns",
+                                            4: "single pixel cell 55um x 500um, high-statistics table", 0: "tiny cell 55um x 50um"}[args.config],
+                              d["nx"], d["ny"], d["nz"], nt, d["dt"], args.tracks, args.carriers),
                            "l2": "inputs larger than L2 (H table %.2f GB, trajectories %.2f GB)" % (n_nodes * nt * 12 / 1e9, n_steps_total * 24 / 1e9),
                            "parallelism": "replicas, tracks sharded" if world > 1 else "single GPU"},
                 "h_solve_s_per_geometry": solve_ms * 1e-3, "step_value": total_terms / (step_ms * 1e-3), "stages": stages,
@@ -453,6 +456,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--tracks", type=int, default=1000, help="MIP tracks per GPU")
     ap.add_argument("--carriers", type=int, default=1000, help="macro-carriers per track")
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 4],
+                    help="BASELINE.json config whose geometry, grid and nt are used (default 1 = the bench line; 2 and 4 are "
+                         "measured as extra rows of BASELINE.md with one batch of tracks, see DESIGN.md)")
     ap.add_argument("--grid", default="", help="override grid, e.g. 32x32x64 (debug only; not a bench line)")
     ap.add_argument("--nt", type=int, default=0, help="override nt (debug only)")
     ap.add_argument("--ref-budget", type=float, default=10.0, help="seconds of oracle work per leg")
