@@ -64,9 +64,13 @@ __device__ __forceinline__ void fft_pass(const C2* __restrict__ in, C2* __restri
   const int per_line = L / R;
   const int total = per_line * n_lines;
   const int tmul = L / (Ns * R);
+  // t / n_lines by a multiply (exact for t * n_lines < 2^32, i.e. any tile that fits in shared memory);
+  // j % Ns by a mask while Ns is a power of two (always, except after a first radix-3 pass)
+  const unsigned inv_lines = 0xffffffffu / (unsigned)n_lines + 1u;
+  const bool ns_pow2 = (Ns & (Ns - 1)) == 0;
   for (int t = threadIdx.x; t < total; t += blockDim.x) {
-    const int j = t / n_lines, line = t - j * n_lines;
-    const int k = j % Ns;
+    const int j = (n_lines == 1) ? t : (int)__umulhi((unsigned)t, inv_lines), line = t - j * n_lines;
+    const int k = ns_pow2 ? (j & (Ns - 1)) : j % Ns;
     const C2* src = in + line * ls;
     C2 v[R];
 #pragma unroll

@@ -233,7 +233,7 @@ Plan make_plan(int nx, int ny, int nz, int L, bool force_generic) {
     p.plane_step = k_plane<false>;
     p.plane_emit = k_plane<true>;
     p.plane_block = dim3(256);
-    p.plane_smem = (size_t)2 * (nx / 2) * (ny + 1) * sizeof(float2);
+    p.plane_smem = (size_t)2 * (nx / 2) * (ny + 1) * sizeof(float2) + (size_t)(nx + ny) * sizeof(float2);
   }
   if (!force_generic) {
     if (nz == 256 && y2 % 8 == 0) set_line<256, 16, 8>(p, nx, y2, L);
@@ -248,7 +248,7 @@ Plan make_plan(int nx, int ny, int nz, int L, bool force_generic) {
     p.line_delta = k_spectral<false, true>;
     p.line_grid = dim3(nx * (y2 / p.ty));
     p.line_block = dim3(32 * p.ty);
-    p.line_smem = (size_t)3 * nz * p.ty * sizeof(float2) + (size_t)std::max(1, L) * p.ty * 32 * sizeof(double2);
+    p.line_smem = (size_t)3 * nz * p.ty * sizeof(float2) + (size_t)std::max(1, L) * p.ty * 32 * sizeof(double2) + (size_t)nz * sizeof(float2);
   }
   return p;
 }

@@ -18,7 +18,6 @@ __global__ void __launch_bounds__(256) k_spectral(const __grid_constant__ GeomBa
   pdl_trigger();
   const GeomDev& g = gb.g[blockIdx.y];
   if (substep >= g.n_sub) { pdl_wait(); return; }
-  pdl_wait();
   const int nx = gd.nx, nz = gd.nz, y2 = gd.y2, TY = gd.ty;
   const int tiles = y2 / TY;
   const int kx = blockIdx.x / tiles, ky0 = (blockIdx.x % tiles) * TY;
@@ -30,6 +29,12 @@ __global__ void __launch_bounds__(256) k_spectral(const __grid_constant__ GeomBa
   float2* b1 = b0 + nelem;
   float2* b2 = b1 + nelem;
   double2* red = reinterpret_cast<double2*>(b2 + nelem);   // [L][TY][32]
+  // twiddles of the z transform: to shared memory while the predecessor runs (every butterfly of every pass
+  // would otherwise fetch them from global memory in the middle of the kernel)
+  float2* s_twz = reinterpret_cast<float2*>(red + (size_t)(L > 0 ? L : 1) * TY * 32);   // [nz]
+  for (int i = tid; i < nz; i += bd) s_twz[i] = g.twz[i];
+  __syncthreads();
+  pdl_wait();
   float2* mV = emit ? g.e0 : g.v0;
   float2* mE = emit ? g.e1 : g.v1;
   const size_t slab = (size_t)kx * nz * y2 + ky0;
@@ -44,9 +49,9 @@ __global__ void __launch_bounds__(256) k_spectral(const __grid_constant__ GeomBa
       b2[t] = g.m2[gi];
     }
     __syncthreads();
-    dres = fft_lines<float2>(b0, b1, nz, TY, 1, TY, g.twz, false);
+    dres = fft_lines<float2>(b0, b1, nz, TY, 1, TY, s_twz, false);
     float2* free1 = (dres == b0) ? b1 : b0;
-    jres = fft_lines<float2>(b2, free1, nz, TY, 1, TY, g.twz, false);
+    jres = fft_lines<float2>(b2, free1, nz, TY, 1, TY, s_twz, false);
     vb = (jres == b2) ? free1 : b2;
   } else {
     vb = b0; dres = b1; jres = b2;
@@ -105,13 +110,13 @@ __global__ void __launch_bounds__(256) k_spectral(const __grid_constant__ GeomBa
     (emit ? g.pl_e : g.pl)[((size_t)l * nx + kx) * y2 + ky0 + j] = s;
   }
   // inverse z transforms
-  float2* vres = fft_lines<float2>(vb, jres, nz, TY, 1, TY, g.twz, true);
+  float2* vres = fft_lines<float2>(vb, jres, nz, TY, 1, TY, s_twz, true);
   float2* fr = (vres == vb) ? jres : vb;
   for (int t = tid; t < nelem; t += bd) {
     const int z = t / TY, tyy = t - z * TY;
     mV[slab + (size_t)z * y2 + tyy] = vres[t];
   }
-  float2* eres = fft_lines<float2>(dres, fr, nz, TY, 1, TY, g.twz, true);
+  float2* eres = fft_lines<float2>(dres, fr, nz, TY, 1, TY, s_twz, true);
   for (int t = tid; t < nelem; t += bd) {
     const int z = t / TY, tyy = t - z * TY;
     mE[slab + (size_t)z * y2 + tyy] = eres[t];
@@ -131,7 +136,6 @@ __global__ void __launch_bounds__(256) k_plane(const __grid_constant__ GeomBatch
   pdl_trigger();
   const GeomDev& g = gb.g[blockIdx.y];
   if (substep >= g.n_sub) { pdl_wait(); return; }
-  pdl_wait();
   const int nx = gd.nx, ny = gd.ny, nz = gd.nz, y2 = gd.y2;
   const int z = blockIdx.x;
   const int tid = threadIdx.x, bd = blockDim.x;
@@ -141,6 +145,13 @@ __global__ void __launch_bounds__(256) k_plane(const __grid_constant__ GeomBatch
   extern __shared__ __align__(16) unsigned char smraw[];
   float2* w1 = reinterpret_cast<float2*>(smraw);
   float2* w2 = w1 + bufsz;
+  // twiddles of the x and y transforms: to shared memory while the predecessor runs
+  float2* s_twx = w2 + bufsz;                              // [nx]
+  float2* s_twy = s_twx + nx;                              // [ny]
+  for (int i = tid; i < nx; i += bd) s_twx[i] = g.twx[i];
+  for (int i = tid; i < ny; i += bd) s_twy[i] = g.twy[i];
+  __syncthreads();
+  pdl_wait();
   const float2* mV = EMIT ? g.e0 : g.v0;
   const float2* mE = EMIT ? g.e1 : g.v1;
   const int L = g.L;
@@ -166,7 +177,7 @@ __global__ void __launch_bounds__(256) k_plane(const __grid_constant__ GeomBatch
       w1[t] = v;
     }
     __syncthreads();
-    float2* r = fft_lines<float2>(w1, w2, nx, y2, 1, y2, g.twx, true);
+    float2* r = fft_lines<float2>(w1, w2, nx, y2, 1, y2, s_twx, true);
     float2* o = (r == w1) ? w2 : w1;
     // pack two x-rows into one complex line with the Hermitian completion along y (Nyquist = 0)
     for (int t = tid; t < nline; t += bd) {
@@ -184,7 +195,7 @@ __global__ void __launch_bounds__(256) k_plane(const __grid_constant__ GeomBatch
       o[p * nyp + k] = zv;
     }
     __syncthreads();
-    float2* e = fft_lines<float2>(o, r, ny, hx, nyp, 1, g.twy, true);
+    float2* e = fft_lines<float2>(o, r, ny, hx, nyp, 1, s_twy, true);
     float2* f = (e == o) ? r : o;
     if (EMIT) {
       // H[n] = E/dt into the staging slot, [slot][comp][z][x][y]
@@ -209,7 +220,7 @@ __global__ void __launch_bounds__(256) k_plane(const __grid_constant__ GeomBatch
       }
     }
     __syncthreads();
-    float2* jf = fft_lines<float2>(e, f, ny, hx, nyp, 1, g.twy, false);
+    float2* jf = fft_lines<float2>(e, f, ny, hx, nyp, 1, s_twy, false);
     float2* jo = (jf == e) ? f : e;
     for (int t = tid; t < hx * y2; t += bd) {
       const int p = t / y2, k = t - p * y2;
@@ -219,7 +230,7 @@ __global__ void __launch_bounds__(256) k_plane(const __grid_constant__ GeomBatch
       jo[(2 * p + 1) * y2 + k] = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
     }
     __syncthreads();
-    float2* jt = fft_lines<float2>(jo, jf, nx, y2, 1, y2, g.twx, false);
+    float2* jt = fft_lines<float2>(jo, jf, nx, y2, 1, y2, s_twx, false);
     for (int t = tid; t < nspec; t += bd) {
       const int kx = t / y2, ky = t - kx * y2;
       const float2 j = jt[t];
