@@ -440,7 +440,7 @@ def run_ours(args):
             o_terms, o_t, o_car = oracle_conv_sample(d, lambda ix, iy, iz: table[(ix, iy, iz)], sample, args.ref_budget)
             per_sub, nsubs, _, _ = oracle_solve_sample(d, args.ref_budget)
             line["cpu_baseline"] = {"value": o_terms / o_t, "unit": UNIT, "cores": 1, "kind": "oracle",
-                                    "sample": "%d carriers of track 0 (%.1f s) for Eq. 1.1; %d Euler substeps on the full grid (%.2f s each) "
+                                    "sample": "first %d carriers (%.1f s) for Eq. 1.1; %d Euler substeps on the full grid (%.2f s each) "
                                               "-> H solve extrapolated to %.0f s per geometry" % (o_car, o_t, nsubs, per_sub, per_sub * n_sub * (nt - 1)),
                                     "h_solve_s_per_geometry_extrapolated": per_sub * n_sub * (nt - 1), "host_cores_available": os.cpu_count()}
         print(json.dumps(line))
