@@ -141,3 +141,16 @@ def test_every_config_geometry_on_a_reduced_grid():
     assert wt.wt_query(geoms[0], wt.WT_Q_SUBSTEPS) == 10 * wt.wt_query(geoms[1], wt.WT_Q_SUBSTEPS)
     for h, d in ((ha, d3a), (hb, d3b)):
         assert wo.h_rel_l2(h, wo.solve_H_from_desc(d)) <= TOL
+
+
+def test_cfg1_full_grid_window_matches_the_oracle():
+    """BASELINE.json configs[1] at its full grid (64x64x256, 370 pad nodes, n_sub = 50) in the launch configuration
+    bench.py times (k_plane_fast<64>, k_pencil2<256>, k_boundary_fast<6,5>, replayed graph): the first 4 time samples
+    (150 Euler substeps) against the oracle, whole table.  The oracle needs about two minutes of one host core."""
+    d = reduced_desc(geometry_desc(1), nt=4)
+    _, (h,) = _solve([d])
+    ref = wo.solve_H_from_desc(d)
+    err = wo.h_rel_l2(h, ref)
+    per_slice = _slice_report(h, ref)
+    assert err <= TOL, (err, per_slice)
+    assert per_slice.max() <= 20 * TOL, per_slice
