@@ -271,9 +271,11 @@ def run_ours(args):
     side = wt._stream(dev)
 
     # ---- inputs (outside the timed region): the table for the drift field, then the trajectories
-    H = [torch.empty((d["nx"], d["ny"], d["nz"], nt, 3), dtype=torch.float32, device=dev)]
-    ws_solve = torch.empty(wt.wt_query(g, wt.WT_Q_SOLVE_WORKSPACE_BYTES) + 256, dtype=torch.uint8, device=dev)
-    wt.wt_solve_H([g], H=H, workspace=ws_solve, device=dev)
+    K = max(1, args.batch)       # lock-step copies of the geometry in one wt_solve_H call (1 = the bench line)
+    gs = [g] * K
+    H = [torch.empty((d["nx"], d["ny"], d["nz"], nt, 3), dtype=torch.float32, device=dev) for _ in range(K)]
+    ws_solve = torch.empty(K * wt.wt_query(g, wt.WT_Q_SOLVE_WORKSPACE_BYTES) + 256, dtype=torch.uint8, device=dev)
+    wt.wt_solve_H(gs, H=H, workspace=ws_solve, device=dev)
     torch.cuda.synchronize()
     e_static = H[0].view(n_nodes, nt, 3).sum(dim=1).mul_(d["dt"]).view(d["nx"], d["ny"], d["nz"], 3)
     theta_max = 15.0 if args.config == 4 else 10.0
@@ -293,7 +295,7 @@ def run_ours(args):
     def step(ev=None):
         if ev:
             ev[0].record(side)
-        wt.wt_solve_H([g], H=H, workspace=ws_solve, device=dev)
+        wt.wt_solve_H(gs, H=H, workspace=ws_solve, device=dev)
         if ev:
             ev[1].record(side)
         wt.wt_convolve_currents(g, H[0], csr["track_carrier_offsets"], csr["carrier_step_offsets"], csr["pos"], csr["vel"],
@@ -382,7 +384,7 @@ def run_ours(args):
         # H solve: 60 N bytes per Euler substep + 40 N per output step, duration = events
         # around wt_solve_H.
         N = n_nodes
-        alg_solve_bytes = (60 * N * n_sub + 40 * N) * (nt - 1) + 40 * N
+        alg_solve_bytes = K * ((60 * N * n_sub + 40 * N) * (nt - 1) + 40 * N)
         conv_gbs = alg_conv_bytes / (conv_ms * 1e-3) / 1e9
         solve_gbs = alg_solve_bytes / (solve_ms * 1e-3) / 1e9
         dominant_is_solve = solve_ms >= conv_ms
@@ -390,7 +392,7 @@ def run_ours(args):
         # solve = 35.9 MB per substep in the cold-cache capture of its three kernels (an upper bound: in the replayed
         # graph the working set is L2-resident); Eq. 1.1 = 154.4 GB per call at 1000 tracks x 1000 carriers.
         default_workload = (args.config == 1 and args.tracks == 1000 and args.carriers == 1000 and not args.grid and not args.nt)
-        traffic_solve = 35.9e6 * n_sub * (nt - 1) if default_workload else None
+        traffic_solve = 35.9e6 * n_sub * (nt - 1) if (default_workload and K == 1) else None
         traffic_conv = 154.4e9 if default_workload else None
         roof = {"bound": "hbm", "kernel": "wt_solve_H (k_plane_fast + k_pencil2 + k_boundary_fast, all substeps)" if dominant_is_solve
                 else "k_conv_systolic", "achieved": solve_gbs if dominant_is_solve else conv_gbs, "peak": peak, "unit": "GB/s",
@@ -400,7 +402,8 @@ def run_ours(args):
         stages = {"solve_ms": solve_ms, "conv_ms": conv_ms,
                   "solve": {"algorithmic_bytes": alg_solve_bytes, "achieved_gbs": solve_gbs, "frac": solve_gbs / peak,
                             "traffic": traffic_solve,
-                            "n_sub": n_sub, "substeps": n_sub * (nt - 1), "us_per_substep": 1e3 * solve_ms / (n_sub * (nt - 1)), "pads": n_pads},
+                            "n_sub": n_sub, "substeps": n_sub * (nt - 1), "us_per_substep": 1e3 * solve_ms / (n_sub * (nt - 1)) / K, "pads": n_pads,
+                            "lock_step_geometries": K},
                   "conv": {"algorithmic_bytes": alg_conv_bytes, "no_reuse_gather_bytes": 96 * terms, "achieved_gbs": conv_gbs,
                            "frac": conv_gbs / peak, "traffic": traffic_conv, "carriers": n_car, "carrier_steps": n_steps_total,
                            "mean_steps": n_steps_total / max(1, n_car)}}
@@ -413,7 +416,7 @@ def run_ours(args):
                               d["nx"], d["ny"], d["nz"], nt, d["dt"], args.tracks, args.carriers),
                            "l2": "inputs larger than L2 (H table %.2f GB, trajectories %.2f GB)" % (n_nodes * nt * 12 / 1e9, n_steps_total * 24 / 1e9),
                            "parallelism": "replicas, tracks sharded" if world > 1 else "single GPU"},
-                "h_solve_s_per_geometry": solve_ms * 1e-3, "step_value": total_terms / (step_ms * 1e-3), "stages": stages,
+                "h_solve_s_per_geometry": solve_ms * 1e-3 / K, "step_value": total_terms / (step_ms * 1e-3), "stages": stages,
                 "roofline": roof,
                 "e2e": {"value": total_terms / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "what": "Eq. 1.1 stage with pinned host trajectories in, host currents out, %d track batches, copies overlapped with the kernels" % n_batches,
@@ -459,6 +462,7 @@ def main():
     ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 4],
                     help="BASELINE.json config whose geometry, grid and nt are used (default 1 = the bench line; 2 and 4 are "
                          "measured as extra rows of BASELINE.md with one batch of tracks, see DESIGN.md)")
+    ap.add_argument("--batch", type=int, default=1, help="lock-step copies of the geometry per wt_solve_H call (extra measurement; 1 = bench line)")
     ap.add_argument("--grid", default="", help="override grid, e.g. 32x32x64 (debug only; not a bench line)")
     ap.add_argument("--nt", type=int, default=0, help="override nt (debug only)")
     ap.add_argument("--ref-budget", type=float, default=10.0, help="seconds of oracle work per leg")
