@@ -76,8 +76,9 @@ def test_cfg0_currents_match_the_oracle():
 
 def test_ragged_and_degenerate_inputs():
     """Empty carriers, a carrier longer than nt (R26), steps outside the box, non-finite steps,
-    a track without carriers, several tiles of outputs (nt = 1024 > 512 per tile) and nt = 4."""
-    for nt in (1024, 4, 36):
+    a track without carriers, nt = 1024 (eight warps per carrier), nt = 1028 (beyond the systolic kernel's range:
+    the one-CTA-per-carrier kernel), nt = 4 and nt = 36 (partly filled last warp)."""
+    for nt in (1024, 1028, 4, 36):
         d = reduced_desc(geometry_desc(0), grid=(12, 8, 6), nt=nt)
         g = wt.wt_make_geometry(d)
         rng = np.random.default_rng(nt)
