@@ -33,7 +33,7 @@ template <int N> struct PlaneCfg {
 // Exchanges ping-pong between two buffers P and Q: six barriers per plane.
 // ------------------------------------------------------------------------------------------------
 template <int N, int E, bool EMIT>
-__global__ void __launch_bounds__(N * N / (2 * E), (N <= 64) ? 4 : 1)
+__global__ void __launch_bounds__(N * N / (2 * E), (N <= 64) ? 3 : 1)   // 80 registers, no spills (4 CTAs/SM at 64 registers spilled and measured 1 us slower per substep)
 k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
   using C = PlaneCfg<N>;
   constexpr int Y2 = C::Y2, T = N / E, SX = C::SX, SU = C::SU, BUF = C::BUF;
