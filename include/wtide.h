@@ -134,10 +134,16 @@ int wt_query(const wt_geometry* geom, int what, int64_t* value);
  *   WT_A_COLUMN_ID     int8   [nx][ny][nz]   column index of the node, -1 = diamond
  *   WT_A_PAD_NODES     int32  [B][3]         (ix, iy, iz) in pad order (column, then ix, iy)
  *   WT_A_PAD_POTENTIAL double [B]
+ *   WT_A_AINV          double [B][B]         upper-left block of the inverse bordered collocation matrix, pad order,
+ *                                            in the library's units (eps = 1, unit voxel): the oracle's block / (eps * voxel volume)
+ *   WT_A_GT, WT_A_GZT  float  [nx][nz][ny/2] mixed-space fundamental solution g~(kx, dz, ky) and its -d/dz
  * `bytes` must be exactly the array size. */
 #define WT_A_COLUMN_ID     1
 #define WT_A_PAD_NODES     2
 #define WT_A_PAD_POTENTIAL 3
+#define WT_A_AINV          4
+#define WT_A_GT            5
+#define WT_A_GZT           6
 int wt_get_array(const wt_geometry* geom, int what, void* host_out, size_t bytes);
 
 /* Number of CUDA kernels this process has launched through libwtide so far (bench.py reports the

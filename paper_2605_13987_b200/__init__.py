@@ -18,7 +18,7 @@ WT_OK, WT_EINVAL, WT_EGEOM, WT_EUNSTABLE, WT_ENOMEM, WT_ECUDA = 0, -1, -2, -3, -
 WT_BIAS, WT_READOUT = 0, 1
 WT_Q_H_BYTES, WT_Q_SOLVE_WORKSPACE_BYTES, WT_Q_SUBSTEPS, WT_Q_N_PADS = 1, 2, 3, 4
 WT_Q_N_NODES, WT_Q_N_CONDUCTING, WT_Q_N_PAD_LAYERS, WT_Q_NT = 5, 6, 7, 8
-WT_A_COLUMN_ID, WT_A_PAD_NODES, WT_A_PAD_POTENTIAL = 1, 2, 3
+WT_A_COLUMN_ID, WT_A_PAD_NODES, WT_A_PAD_POTENTIAL, WT_A_AINV, WT_A_GT, WT_A_GZT = 1, 2, 3, 4, 5, 6
 
 EXPORTS = ("wt_make_geometry", "wt_solve_H", "wt_convolve_currents", "wt_free", "wt_trajectory_nodes",
            "wt_conv_workspace_bytes", "wt_query", "wt_get_array", "wt_last_error", "wt_launch_count")
@@ -50,6 +50,8 @@ def _load():
         except Exception as e:  # noqa: BLE001
             if not os.path.exists(path):
                 raise ImportError(f"libwtide.so is missing and could not be built with nvcc: {e}") from e
+            import warnings
+            warnings.warn(f"libwtide.so is older than its sources and the nvcc rebuild failed ({e}); loading the STALE library")
     lib = C.CDLL(path)
     vp, i64, sz = C.c_void_p, C.c_int64, C.c_size_t
     lib.wt_make_geometry.argtypes = [C.POINTER(wt_geometry_desc), C.POINTER(vp)]
@@ -131,6 +133,10 @@ def wt_get_array(geom: Geometry, what: int) -> np.ndarray:
         a = np.empty((nb, 3), np.int32)
     elif what == WT_A_PAD_POTENTIAL:
         a = np.empty(nb, np.float64)
+    elif what == WT_A_AINV:
+        a = np.empty((nb, nb), np.float64)
+    elif what in (WT_A_GT, WT_A_GZT):
+        a = np.empty((nx, nz, ny // 2), np.float32)
     else:
         raise ValueError("unknown array")
     _check(_lib.wt_get_array(geom.handle, what, a.ctypes.data, a.nbytes))

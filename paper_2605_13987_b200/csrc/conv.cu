@@ -385,6 +385,8 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
   }
   if (n_carriers > 0x7fffffffLL || n_tracks > 0x7fffffffLL) { wt_set_error("wt_convolve_currents: more than 2^31-1 carriers or tracks in one call"); return WT_EINVAL; }
   if ((size_t)g->nx * g->ny * g->nz > 0xffffffffull) { wt_set_error("wt_convolve_currents: grid too large"); return WT_EINVAL; }
+  if (((uintptr_t)H_dev) % 16 != 0) { wt_set_error("wt_convolve_currents: H table not 16-byte aligned (rows are read with 128-bit loads)"); return WT_EINVAL; }
+  if (workspace_dev && ((uintptr_t)workspace_dev) % 256 != 0) { wt_set_error("wt_convolve_currents: workspace not 256-byte aligned"); return WT_EINVAL; }
   size_t need = 0;
   wt_conv_workspace_bytes(g, n_tracks, n_carriers, per_track, &need);
   if (need > 0 && (!workspace_dev || workspace_bytes < need)) {
@@ -398,7 +400,7 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
   p.invx = (float)((double)g->nx / g->lx); p.invy = (float)((double)g->ny / g->ly); p.invz = (float)((double)g->nz / g->lz);
   p.dt_over_vw = (float)(g->dt / g->v_w);
   // kernel choice: the systolic kernel for nt <= 1024 (its per-warp rows fit in shared memory), else one CTA per carrier
-  static const bool force_v1 = env_flag("WTIDE_CONV_V1");
+  const bool force_v1 = env_flag("WTIDE_CONV_V1");   // (read per call, like the switches of wt_solve_H)
   const int nw = (g->nt + 127) / 128;
   int gc = 1, stride = 1;
   if (n_carriers > 0 && nw <= 8 && !force_v1) {

@@ -8,7 +8,10 @@
 
 #include <algorithm>
 #include <cmath>
+#include <complex>
+#include <cstdlib>
 #include <cstring>
+#include <thread>
 
 static thread_local std::string g_err;
 std::atomic<long long> g_wt_launches{0};
@@ -39,47 +42,147 @@ inline int mode_of(int k, int n, bool* removed) {
   return (2 * k < n) ? k : k - n;
 }
 
-// Inverse of a dense matrix by LU with partial pivoting (Doolittle), fp64.  Returns false if singular.
-bool invert(std::vector<double>& a, int n, std::vector<double>& inv) {
-  std::vector<int> piv(n);
-  for (int i = 0; i < n; ++i) piv[i] = i;
-  for (int c = 0; c < n; ++c) {
-    int p = c;
-    double best = std::fabs(a[(size_t)c * n + c]);
-    for (int r = c + 1; r < n; ++r) {
-      double v = std::fabs(a[(size_t)r * n + c]);
-      if (v > best) { best = v; p = r; }
-    }
-    if (best == 0.0) return false;
-    if (p != c) {
-      for (int j = 0; j < n; ++j) std::swap(a[(size_t)p * n + j], a[(size_t)c * n + j]);
-      std::swap(piv[p], piv[c]);
-    }
-    double d = 1.0 / a[(size_t)c * n + c];
-    for (int r = c + 1; r < n; ++r) {
-      double f = a[(size_t)r * n + c] * d;
-      a[(size_t)r * n + c] = f;
-      if (f != 0.0)
-        for (int j = c + 1; j < n; ++j) a[(size_t)r * n + j] -= f * a[(size_t)c * n + j];
-    }
+// Runs fn(t, n_threads) on n_threads host threads (t = 0 runs on the caller).
+template <typename F>
+void parallel_run(int n_threads, F fn) {
+  if (n_threads <= 1) { fn(0, 1); return; }
+  std::vector<std::thread> th;
+  th.reserve(n_threads - 1);
+  for (int t = 1; t < n_threads; ++t) th.emplace_back([&fn, t, n_threads] { fn(t, n_threads); });
+  fn(0, n_threads);
+  for (auto& x : th) x.join();
+}
+
+int host_threads(size_t work) {
+  if (work < (size_t)1 << 22) return 1;
+  unsigned hc = std::thread::hardware_concurrency();
+  if (hc == 0) hc = 1;
+  if (const char* e = std::getenv("WTIDE_HOST_THREADS")) hc = (unsigned)std::max(1, std::atoi(e));
+  return (int)std::min(hc, 32u);
+}
+
+// c[0..n) -= f * r[0..n): the inner loop of the elimination (contiguous, vectorised per ISA at load time)
+__attribute__((target_clones("arch=skylake-avx512", "arch=haswell", "default")))
+void row_axpy4(double* __restrict__ c, const double* __restrict__ r0, const double* __restrict__ r1, const double* __restrict__ r2,
+               const double* __restrict__ r3, double f0, double f1, double f2, double f3, int n) {
+  for (int j = 0; j < n; ++j) c[j] -= f0 * r0[j] + f1 * r1[j] + f2 * r2[j] + f3 * r3[j];
+}
+// the same for two rows c, d at once (the four pivot rows are loaded once for both)
+__attribute__((target_clones("arch=skylake-avx512", "arch=haswell", "default")))
+void row_axpy4x2(double* __restrict__ c, double* __restrict__ d, const double* __restrict__ r0, const double* __restrict__ r1,
+                 const double* __restrict__ r2, const double* __restrict__ r3, const double* __restrict__ f, const double* __restrict__ h, int n) {
+  const double f0 = f[0], f1 = f[1], f2 = f[2], f3 = f[3], h0 = h[0], h1 = h[1], h2 = h[2], h3 = h[3];
+  for (int j = 0; j < n; ++j) {
+    const double a0 = r0[j], a1 = r1[j], a2 = r2[j], a3 = r3[j];
+    c[j] -= f0 * a0 + f1 * a1 + f2 * a2 + f3 * a3;
+    d[j] -= h0 * a0 + h1 * a1 + h2 * a2 + h3 * a3;
   }
-  inv.assign((size_t)n * n, 0.0);
-  std::vector<double> col(n);
-  for (int e = 0; e < n; ++e) {
-    for (int i = 0; i < n; ++i) col[i] = (piv[i] == e) ? 1.0 : 0.0;
-    for (int i = 0; i < n; ++i) {          // L y = P e
-      double s = col[i];
-      for (int j = 0; j < i; ++j) s -= a[(size_t)i * n + j] * col[j];
-      col[i] = s;
+}
+
+// In-place inverse of a symmetric positive definite matrix (row-major, n x n) by blocked Gauss-Jordan
+// elimination without pivoting (stable for SPD matrices: it is the elimination order of an LDL^T
+// factorisation), the rank-NB updates of the other rows spread over the host threads.
+// Returns false if a pivot is not positive (matrix not numerically SPD).
+bool invert_spd(std::vector<double>& a, int n) {
+  constexpr int NB = 64;
+  const int n_thr = host_threads((size_t)n * n * n / 8);
+  std::vector<double> rowblk((size_t)NB * n), dinv((size_t)NB * NB), colblk((size_t)n * NB);
+  for (int k0 = 0; k0 < n; k0 += NB) {
+    const int nb = std::min(NB, n - k0);
+    // invert the diagonal block (unblocked Gauss-Jordan, no pivoting)
+    for (int i = 0; i < nb; ++i)
+      for (int j = 0; j < nb; ++j) dinv[i * NB + j] = a[(size_t)(k0 + i) * n + k0 + j];
+    for (int c = 0; c < nb; ++c) {
+      const double piv = dinv[c * NB + c];
+      if (!(piv > 0.0) || !std::isfinite(piv)) return false;
+      const double d = 1.0 / piv;
+      dinv[c * NB + c] = 1.0;
+      for (int j = 0; j < nb; ++j) dinv[c * NB + j] *= d;
+      for (int r = 0; r < nb; ++r) {
+        if (r == c) continue;
+        const double f = dinv[r * NB + c];
+        dinv[r * NB + c] = 0.0;
+        for (int j = 0; j < nb; ++j) dinv[r * NB + j] -= f * dinv[c * NB + j];
+      }
     }
-    for (int i = n - 1; i >= 0; --i) {     // U x = y
-      double s = col[i];
-      for (int j = i + 1; j < n; ++j) s -= a[(size_t)i * n + j] * col[j];
-      col[i] = s / a[(size_t)i * n + i];
-    }
-    for (int i = 0; i < n; ++i) inv[(size_t)i * n + e] = col[i];
+    // pivot rows R = D^-1 A[k,:] with the block column replaced by D^-1; keep the old block column of all rows
+    parallel_run(std::min(n_thr, nb), [&](int t, int nt_) {
+      for (int i = t; i < nb; i += nt_) {
+        double* out = &rowblk[(size_t)i * n];
+        for (int j = 0; j < n; ++j) out[j] = 0.0;
+        for (int p = 0; p < nb; ++p) {
+          const double f = dinv[i * NB + p];
+          const double* src = &a[(size_t)(k0 + p) * n];
+          for (int j = 0; j < n; ++j) out[j] += f * src[j];
+        }
+        for (int j = 0; j < nb; ++j) out[k0 + j] = dinv[i * NB + j];
+      }
+    });
+    for (int r = 0; r < n; ++r)
+      for (int p = 0; p < nb; ++p) { colblk[(size_t)r * NB + p] = a[(size_t)r * n + k0 + p]; }
+    // every other row: A[r,:] -= A[r,k] R, with its block column set to -A[r,k] D^-1
+    parallel_run(n_thr, [&](int t, int nt_) {
+      auto one_row = [&](int r) {
+        double* c = &a[(size_t)r * n];
+        const double* f = &colblk[(size_t)r * NB];
+        for (int p = 0; p < nb; ++p) c[k0 + p] = 0.0;
+        int p = 0;
+        for (; p + 3 < nb; p += 4)
+          row_axpy4(c, &rowblk[(size_t)p * n], &rowblk[(size_t)(p + 1) * n], &rowblk[(size_t)(p + 2) * n], &rowblk[(size_t)(p + 3) * n],
+                    f[p], f[p + 1], f[p + 2], f[p + 3], n);
+        for (; p < nb; ++p) {
+          const double fp = f[p];
+          const double* rr = &rowblk[(size_t)p * n];
+          for (int j = 0; j < n; ++j) c[j] -= fp * rr[j];
+        }
+      };
+      // rows in pairs (2 t, 2 t + 1), (2 t + 2 nt_, ...): a pair that touches the pivot block falls back to single rows
+      for (int r = 2 * t; r < n; r += 2 * nt_) {
+        const int r2 = r + 1;
+        const bool in0 = (r >= k0 && r < k0 + nb), in1 = (r2 >= n) || (r2 >= k0 && r2 < k0 + nb);
+        if (in0 || in1 || nb % 4 != 0) {
+          if (!in0) one_row(r);
+          if (r2 < n && !(r2 >= k0 && r2 < k0 + nb)) one_row(r2);
+          continue;
+        }
+        double* c = &a[(size_t)r * n];
+        double* d = &a[(size_t)r2 * n];
+        const double* f = &colblk[(size_t)r * NB];
+        const double* h = &colblk[(size_t)r2 * NB];
+        for (int p = 0; p < nb; ++p) { c[k0 + p] = 0.0; d[k0 + p] = 0.0; }
+        for (int p = 0; p < nb; p += 4)
+          row_axpy4x2(c, d, &rowblk[(size_t)p * n], &rowblk[(size_t)(p + 1) * n], &rowblk[(size_t)(p + 2) * n],
+                      &rowblk[(size_t)(p + 3) * n], f + p, h + p, n);
+      }
+    });
+    for (int i = 0; i < nb; ++i) std::memcpy(&a[(size_t)(k0 + i) * n], &rowblk[(size_t)i * n], (size_t)n * sizeof(double));
   }
   return true;
+}
+
+// In-place complex DFT of length n = 2^a 3^b (fp64, e^{+2 pi i jk/n}), recursive decimation in time with a
+// twiddle table tw[k] = e^{+2 pi i k/n_top}; `stride` = n_top / n.  Used for the z-sums of the fundamental solution.
+void dft_rec(std::complex<double>* x, std::complex<double>* tmp, int n, int stride, const std::complex<double>* tw) {
+  if (n == 1) return;
+  const int r = (n % 2 == 0) ? 2 : 3, m = n / r;
+  // split into r interleaved subsequences, transform each
+  for (int q = 0; q < r; ++q)
+    for (int j = 0; j < m; ++j) tmp[q * m + j] = x[j * r + q];
+  for (int q = 0; q < r; ++q) dft_rec(tmp + q * m, x, m, stride * r, tw);   // (x serves as scratch)
+  if (r == 2) {
+    for (int k = 0; k < m; ++k) {
+      const std::complex<double> e = tmp[k], o = tmp[m + k] * tw[(size_t)k * stride];
+      x[k] = e + o; x[k + m] = e - o;
+    }
+  } else {
+    const std::complex<double> w3 = tw[(size_t)m * stride], w32 = tw[(size_t)2 * m * stride];   // e^{2 pi i/3}, e^{4 pi i/3}
+    for (int k = 0; k < m; ++k) {
+      const std::complex<double> a0 = tmp[k], a1 = tmp[m + k] * tw[(size_t)k * stride], a2 = tmp[2 * m + k] * tw[(size_t)2 * k * stride];
+      x[k] = a0 + a1 + a2;
+      x[k + m] = a0 + w3 * a1 + w32 * a2;
+      x[k + 2 * m] = a0 + w32 * a1 + w3 * a2;
+    }
+  }
 }
 }  // namespace
 
@@ -208,34 +311,35 @@ extern "C" int wt_make_geometry(const wt_geometry_desc* d, wt_geometry** out) {
   //   gt (kx,ky,dz) = sum_kz cos(2 pi m_z dz/nz) / |kappa|^2
   //   gzt(kx,ky,dz) = sum_kz kappa_z sin(2 pi m_z dz/nz) / |kappa|^2     (= -d/dz of gt)
   // over retained kz with (kx,ky,kz) != 0.  Layout [kx][dz][ky].
+  // Per (kx, ky) these are the real and imaginary part of ONE length-nz DFT of the real sequence w + w kappa_z
+  // (w = 1/|kappa|^2 is even in kz, w kappa_z is odd), O(N log nz) in total instead of O(N nz); lines over host threads.
   g->gt.assign((size_t)nx * nz * y2, 0.0f);
   g->gzt.assign((size_t)nx * nz * y2, 0.0f);
   std::vector<double> gt64((size_t)nx * nz * y2, 0.0);   // kept in fp64 for the collocation matrix
-  std::vector<double> cs(nz), sn(nz);
-  for (int i = 0; i < nz; ++i) { cs[i] = std::cos(2.0 * kPi * i / nz); sn[i] = std::sin(2.0 * kPi * i / nz); }
-  std::vector<double> w(nz);
-  for (int ikx = 0; ikx < nx; ++ikx) {
-    if (!rx[ikx]) continue;
-    for (int iky = 0; iky < y2; ++iky) {
-      const double kxy2 = g->kx[ikx] * g->kx[ikx] + g->ky[iky] * g->ky[iky];
-      for (int ikz = 0; ikz < nz; ++ikz) {
-        double k2 = kxy2 + g->kz[ikz] * g->kz[ikz];
-        w[ikz] = (rz[ikz] && k2 > 0.0) ? 1.0 / k2 : 0.0;
-      }
-      for (int dz = 0; dz < nz; ++dz) {
-        double a = 0.0, b = 0.0;
-        for (int ikz = 0; ikz < nz; ++ikz) {
-          if (w[ikz] == 0.0) continue;
-          int ph = (int)(((int64_t)ikz * dz) % nz);        // e^{i kappa_z z}: index k and mode m give the same phase
-          a += w[ikz] * cs[ph];
-          b += w[ikz] * g->kz[ikz] * sn[ph];
+  {
+    std::vector<std::complex<double>> tw(nz);
+    for (int i = 0; i < nz; ++i) tw[i] = std::complex<double>(std::cos(2.0 * kPi * i / nz), std::sin(2.0 * kPi * i / nz));
+    parallel_run(host_threads(N * 8), [&](int t, int nt_) {
+      std::vector<std::complex<double>> line(nz), tmp(nz);
+      for (int ikx = t; ikx < nx; ikx += nt_) {
+        if (!rx[ikx]) continue;
+        for (int iky = 0; iky < y2; ++iky) {
+          const double kxy2 = g->kx[ikx] * g->kx[ikx] + g->ky[iky] * g->ky[iky];
+          for (int ikz = 0; ikz < nz; ++ikz) {
+            const double k2 = kxy2 + g->kz[ikz] * g->kz[ikz];
+            const double w = (rz[ikz] && k2 > 0.0) ? 1.0 / k2 : 0.0;
+            line[ikz] = std::complex<double>(w + w * g->kz[ikz], 0.0);
+          }
+          dft_rec(line.data(), tmp.data(), nz, 1, tw.data());
+          for (int dz = 0; dz < nz; ++dz) {
+            const size_t o = ((size_t)ikx * nz + dz) * y2 + iky;
+            gt64[o] = line[dz].real();
+            g->gt[o] = (float)line[dz].real();
+            g->gzt[o] = (float)line[dz].imag();
+          }
         }
-        size_t o = ((size_t)ikx * nz + dz) * y2 + iky;
-        gt64[o] = a;
-        g->gt[o] = (float)a;
-        g->gzt[o] = (float)b;
       }
-    }
+    });
   }
 
   // ---- bordered collocation matrix (step 4; R10) in eps = 1 units -----------------------------------
@@ -269,23 +373,31 @@ extern "C" int wt_make_geometry(const wt_geometry_desc* d, wt_geometry** out) {
           planes[p][(size_t)dx * ny + dy] = s / (double)N;
         }
     }
-    const int n = B + 1;
-    std::vector<double> a((size_t)n * n, 0.0), inv;
-    for (int i = 0; i < B; ++i) {
+    // Upper-left B x B block of the inverse of [[G,1],[1^T,0]] by the Schur complement of the SPD Green block:
+    //   Ainv_BB = G^-1 - u u^T / (1^T u),  u = G^-1 1       (the constant c is never used, R33)
+    std::vector<double> a((size_t)B * B);
+    for (int i = 0; i < B; ++i)
       for (int j = 0; j < B; ++j) {
         int ddx = ((g->pad_nodes[3 * i] - g->pad_nodes[3 * j]) % nx + nx) % nx;
         int ddy = ((g->pad_nodes[3 * i + 1] - g->pad_nodes[3 * j + 1]) % ny + ny) % ny;
         int ddz = ((g->pad_nodes[3 * i + 2] - g->pad_nodes[3 * j + 2]) % nz + nz) % nz;
         size_t p = std::find(dz_list.begin(), dz_list.end(), ddz) - dz_list.begin();
-        a[(size_t)i * n + j] = planes[p][(size_t)ddx * ny + ddy];
+        a[(size_t)i * B + j] = planes[p][(size_t)ddx * ny + ddy];
       }
-      a[(size_t)i * n + B] = 1.0;
-      a[(size_t)B * n + i] = 1.0;
+    if (!invert_spd(a, B)) { delete g; wt_set_error("wt_make_geometry: singular collocation matrix (Green block not positive definite)"); return WT_EGEOM; }
+    std::vector<double> u(B, 0.0);
+    double ssum = 0.0;
+    for (int i = 0; i < B; ++i) {
+      double s = 0.0;
+      for (int j = 0; j < B; ++j) s += a[(size_t)i * B + j];
+      u[i] = s; ssum += s;
     }
-    if (!invert(a, n, inv)) { delete g; wt_set_error("wt_make_geometry: singular collocation matrix"); return WT_EGEOM; }
+    if (!(ssum != 0.0) || !std::isfinite(ssum)) { delete g; wt_set_error("wt_make_geometry: singular collocation matrix"); return WT_EGEOM; }
     g->ainv.resize((size_t)B * B);
-    for (int i = 0; i < B; ++i)
-      for (int j = 0; j < B; ++j) g->ainv[(size_t)i * B + j] = inv[(size_t)i * n + j];
+    for (int i = 0; i < B; ++i) {
+      const double ui = u[i] / ssum;
+      for (int j = 0; j < B; ++j) g->ainv[(size_t)i * B + j] = a[(size_t)i * B + j] - ui * u[j];
+    }
   }
   *out = g;
   wt_set_error("");
@@ -308,6 +420,9 @@ extern "C" int wt_get_array(const wt_geometry* g, int what, void* host_out, size
     case WT_A_COLUMN_ID: src = g->col_id.data(); need = g->col_id.size(); break;
     case WT_A_PAD_NODES: src = g->pad_nodes.data(); need = g->pad_nodes.size() * sizeof(int32_t); break;
     case WT_A_PAD_POTENTIAL: src = g->pad_pot.data(); need = g->pad_pot.size() * sizeof(double); break;
+    case WT_A_AINV: src = g->ainv.data(); need = g->ainv.size() * sizeof(double); break;
+    case WT_A_GT: src = g->gt.data(); need = g->gt.size() * sizeof(float); break;
+    case WT_A_GZT: src = g->gzt.data(); need = g->gzt.size() * sizeof(float); break;
     default: wt_set_error("wt_get_array: unknown array"); return WT_EINVAL;
   }
   if (bytes != need) { wt_set_error("wt_get_array: size mismatch, need " + std::to_string(need)); return WT_EINVAL; }

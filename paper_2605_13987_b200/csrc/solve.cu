@@ -412,7 +412,9 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   }
   int* dstep = (int*)(base + off);
   gd.step = dstep;
+#ifdef WTIDE_DEBUG
   gd.stamps = env_flag("WTIDE_STAMPS") ? (long long*)(base + off + 256) : nullptr;
+#endif
   CK(cudaMemsetAsync(dstep, 0, sizeof(int), st));
   // descriptors in launch batches of kBatch geometries
   const int n_batches = (n_geoms + kBatch - 1) / kBatch;
@@ -439,7 +441,11 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   const int bnd_units3 = std::max(1, maxL) * ((nx + kBndKx - 1) / kBndKx);
   const int bnd_rows = (maxB + kBndThreads / 32 - 1) / (kBndThreads / 32);
 
+#ifdef WTIDE_DEBUG   // timing experiments only (drops kernels from the substep loop: WRONG results); never in the shipped library
   const int dbg_skip = std::getenv("WTIDE_DBG_SKIP") ? std::atoi(std::getenv("WTIDE_DBG_SKIP")) : 0;
+#else
+  constexpr int dbg_skip = 0;
+#endif
   const bool pdl = !env_flag("WTIDE_NO_PDL");
   long long launches = 0;
   cudaError_t launch_err = cudaSuccess;

@@ -21,8 +21,12 @@
 
 namespace wt {
 
-// debug (WTIDE_STAMPS=1): clock stamps of thread 0 of each CTA of geometry 0
+// clock stamps of thread 0 of each CTA of geometry 0: only in -DWTIDE_DEBUG builds (never in the shipped library)
+#ifdef WTIDE_DEBUG
 #define WT_STAMP(k) do { if (gd.stamps && threadIdx.x == 0 && blockIdx.y == 0) gd.stamps[blockIdx.x * 16 + (k)] = clock64(); } while (0)
+#else
+#define WT_STAMP(k) do { } while (0)
+#endif
 
 constexpr int kBndCluster = 8;
 constexpr int kBndThreads = 512;

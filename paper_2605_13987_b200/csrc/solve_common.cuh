@@ -14,7 +14,9 @@ struct GridDev {
   int nx, ny, nz, y2, nt, ty, n_tiles;   // generic k_spectral: ty lines per CTA, n_tiles = nx * (y2/ty)
   double inv_n;
   const int* step;                        // device counter: index n of the output step being produced
-  long long* stamps;                      // debug (WTIDE_STAMPS=1): [16 ranks][16] clock stamps of the boundary kernel, else NULL
+#ifdef WTIDE_DEBUG
+  long long* stamps;                      // -DWTIDE_DEBUG builds with WTIDE_STAMPS=1: [16 ranks][16] clock stamps of the boundary kernel, else NULL
+#endif
 };
 
 // One geometry of the lock-step batch.  Passed BY VALUE inside GeomBatch (kernel parameter space =

@@ -181,3 +181,53 @@ def test_many_carriers_ragged_tracks_grouped_path():
     assert np.abs(got_t - ref_t).max() <= TOL * np.abs(ref_t).max()
     empty = np.nonzero(np.diff(toff) == 0)[0]
     assert len(empty) >= 3 and (got_t[empty] == 0).all()
+
+
+@pytest.mark.parametrize("config", [2, 4])
+def test_tables_beyond_2_31_floats_sampled_tracks(config):
+    """BASELINE.json configs[2] (128x128x256, nt = 1024: 51.5 GB, 1.29e10 floats) and configs[4] (96x96x384, nt = 1024:
+    43.5 GB) table sizes in the launch configuration bench.py times (eight warps per carrier): row offsets beyond 2^31
+    floats / 2^32 bytes.  Tracks are placed so that the highest node indices of the table are read; the oracle computes
+    them from rows fetched on demand from the same fp32 table."""
+    d = geometry_desc(config)
+    nx, ny, nz, nt = d["nx"], d["ny"], d["nz"], d["nt"]
+    g2 = wt.wt_make_geometry(d)
+    H = torch.empty((nx, ny, nz, nt, 3), dtype=torch.float32, device=DEV)
+    flat = H.view(-1)
+    gen = torch.Generator(device=DEV).manual_seed(11 + config)
+    step = 1 << 28
+    for a in range(0, flat.numel(), step):
+        flat[a:a + step].normal_(generator=gen)
+    assert flat.numel() > 2 ** 31
+    rng = np.random.default_rng(13 + config)
+    n_car = 24
+    lens = rng.integers(1, 120, size=n_car)
+    lens[3] = nt + 5                                  # longer than the table's time axis (R26)
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    # starts spread over the box, half of them in the last x-planes (node index close to nx*ny*nz)
+    start = np.stack([rng.uniform(0, d["lx"], n_car), rng.uniform(0, d["ly"], n_car), rng.uniform(0, d["lz"], n_car)], axis=1)
+    start[::2, 0] = d["lx"] * (1.0 - rng.uniform(0, 2.5 / nx, size=len(start[::2])))
+    start[::4, 1] = d["ly"] * (1.0 - rng.uniform(0, 2.5 / ny, size=len(start[::4])))
+    start[::4, 2] = d["lz"] * (1.0 - rng.uniform(0, 2.5 / nz, size=len(start[::4])))
+    pos = np.concatenate([start[c] + np.cumsum(rng.normal(0.0, 0.4, size=(lens[c], 3)), axis=0) for c in range(n_car)]).astype(np.float32)
+    vel = (rng.standard_normal((int(off[-1]), 3)) * 100).astype(np.float32)
+    csr = dict(track_carrier_offsets=np.array([0, 5, 5, 17, n_car], np.int64), carrier_step_offsets=off, pos=pos, vel=vel,
+               charge=rng.standard_normal(n_car).astype(np.float32))
+    i0, i1, _, _ = wo.trajectory_nodes((nx, ny, nz), (d["lx"], d["ly"], d["lz"]), pos)
+    top = ((i1[:, 0] * ny + i1[:, 1]) * nz + i1[:, 2]).max()
+    assert top * nt * 3 > 2 ** 31 and top >= nx * ny * nz - 3 * ny * nz
+    cache = {}
+
+    def rows(ix, iy, iz):
+        key = (ix, iy, iz)
+        if key not in cache:
+            cache[key] = H[ix, iy, iz].cpu().numpy()
+        return cache[key]
+    for per_track in (True, False):
+        got = _run(g2, H, csr, per_track)
+        ref = _oracle(d, rows, csr, per_track)
+        l2, mx = wo.current_error(got, ref)
+        assert np.isfinite(got).all()
+        assert l2 <= TOL and mx <= 5 * TOL, (config, per_track, l2, mx)
+    del H
+    torch.cuda.empty_cache()
