@@ -146,6 +146,10 @@ int wt_query(const wt_geometry* geom, int what, int64_t* value);
 #define WT_A_GZT           6
 int wt_get_array(const wt_geometry* geom, int what, void* host_out, size_t bytes);
 
+/* One line naming the execution wt_solve_H selects for this geometry on the current device (persistent kernel or
+ * kernel chain, and which kernels), for logs and bench labels.  Needs no GPU for the chain; `out` is NUL-terminated. */
+int wt_describe_plan(const wt_geometry* geom, char* out, size_t out_bytes);
+
 /* Number of CUDA kernels this process has launched through libwtide so far (bench.py reports the
  * difference over its timed region as "gpu_launches"). */
 int64_t wt_launch_count(void);

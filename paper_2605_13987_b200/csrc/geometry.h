@@ -2,6 +2,7 @@
 #pragma once
 #include <atomic>
 #include <cstdint>
+#include <memory>
 #include <string>
 #include <vector>
 
@@ -31,6 +32,7 @@ struct wt_geometry {
   std::vector<float> gt, gzt;       // [kx][dz][ky] mixed-space fundamental solution and its -d/dz
   std::vector<double> ainv;         // [B][B] upper-left block of the inverse bordered matrix
   std::vector<double> kx, ky, kz;   // wavenumbers (0 at the removed Nyquist index); ky has ny/2 entries
+  std::shared_ptr<void> solve_cache;   // what wt_solve_H derives from the handle on its first call (solve.cu: SolveCache)
 };
 
 extern std::atomic<long long> g_wt_launches;   // kernels launched by this process (wt_launch_count)

@@ -1,0 +1,648 @@
+// Persistent solver of wt_solve_H: ONE cooperative launch per output step of H (n_sub Euler substeps +
+// the emit of H[n]) for one geometry, one CTA per SM, phases separated by grid barriers instead of
+// kernel boundaries (the per-substep kernel chain of solve_chain.cu pays a launch, a first-load round trip
+// and a store drain three times per substep: profiles/r1_solve.md).
+//
+// Method as in solve.cu (Fig. 3 :109; R1-R20).  One Euler substep =
+//   plane phase   all CTAs: (z, component) units, E~ = -i kappa V~ (a5), inverse xy DFT, J = s dt_int E (a6),
+//                 forward xy DFT, i kx J~x, i ky J~y, J~z                                           -> m0, m1, m2
+//   -- grid barrier --
+//   z-line phase  Z CTAs own fixed tiles of z-lines (kx, TYL ky):
+//      pass A     forward z DFT; r^ -= D^ + i kz J^z (a7, fp64 state); V^_rho = r^/|kappa|^2 (a2); potentials of
+//                 the pad layers (fp64) and from them this CTA's contribution to V_rho at EVERY pad node (a3)
+//      boundary   B CTAs (the SMs the z-lines leave idle): rhs = V_pad - sum of the contributions;
+//                 Q' = Ainv rhs: "adjusted, in magnitude, to enforce the boundary conditions"
+//      pass B     spectrum of the boundary point charges for the CTA's own lines; V^ = (r^ + Q^)/|kappa|^2, i.e. the
+//                 translated fundamental solutions of PAPER.md:97 summed in spectral space, in fp64 (a4);
+//                 inverse z DFT of V^ and -i kz V^                                                  -> v0, v1
+//   -- grid barrier --
+// and every n_sub substeps the same phases run on the increment r^ - r^_prev with the pads at 0 V and write
+// H[n] = E/dt (a8) into the staging buffer, which a last phase transposes into the time-innermost table.
+// Spins (grid barrier, boundary hand-over) are bounded: on a time-out the kernel sets ctl->abort, every CTA
+// leaves, later launches return at once and k_persist_finish poisons the table with NaN -- a wrong launch
+// configuration can cost a second, never a hang.
+#pragma once
+#include <type_traits>
+
+#include "solve_fast.cuh"
+
+namespace wt {
+
+struct PersistCtl {                 // device control block, zeroed before the first launch of a solve
+  unsigned long long bar;           // grid-barrier arrivals (monotonic)
+  unsigned long long cnt_part;      // Z CTAs that have published their pad contributions (monotonic)
+  unsigned long long cnt_rhs;       // B CTAs that have published their slice of rhs
+  unsigned long long cnt_q;         // B CTAs that have published their slice of Q'
+  int abort;
+};
+
+struct PersistArgs {
+  GeomDev g;
+  GridDev gd;
+  PersistCtl* ctl;
+  double* part;                     // [B][part_stride]: contribution of Z CTA c to V_rho at pad b
+  const int* pad_x;                 // [B] group order
+  const int* pad_l;                 // [B] layer index of the pad
+  int lpoff[kMaxLayers + 1];        // pads of layer l = [lpoff[l], lpoff[l+1])
+  int n_z_cta, n_b_cta, part_stride;
+  int ainv_in_smem;                 // the B CTA's rows of Ainv live in shared memory for the whole launch
+  unsigned smem_ainv_off;           // byte offset of that slice in the dynamic shared memory
+  int step;                         // index n of the output step this launch produces
+  int n_sub;                        // Euler substeps before the emit (0 for n = 0)
+  unsigned long long bar0, epi0;    // grid barriers / boundary episodes completed by earlier launches
+};
+
+constexpr long long kSpinLimit = 4000000000LL;     // cycles (about two seconds)
+constexpr int kPersistThreads = 512;
+
+__device__ __forceinline__ void group_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
+  unsigned long long v;
+  asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+// thread 0 of a CTA: wait until *ctr >= target; false on time-out / abort
+__device__ __forceinline__ bool spin_until(const unsigned long long* ctr, unsigned long long target, int* abort_flag) {
+  const long long t0 = clock64();
+  unsigned it = 0;
+  while (ld_acquire_u64(ctr) < target) {
+    if ((++it & 63u) == 0) {
+      if (*reinterpret_cast<volatile int*>(abort_flag)) return false;
+      if (clock64() - t0 > kSpinLimit) { atomicExch(abort_flag, 1); return false; }
+    }
+  }
+  return true;
+}
+// publish: everything this CTA wrote before is visible to whoever observes the increment
+__device__ __forceinline__ void cta_signal(unsigned long long* ctr) {
+  __syncthreads();
+  if (threadIdx.x == 0) { __threadfence(); atomicAdd(ctr, 1ULL); }
+}
+__device__ __forceinline__ bool cta_wait(const unsigned long long* ctr, unsigned long long target, int* abort_flag, int* s_ok) {
+  if (threadIdx.x == 0) *s_ok = spin_until(ctr, target, abort_flag) ? 1 : 0;
+  __syncthreads();
+  const bool ok = *s_ok != 0;
+  __syncthreads();
+  return ok;
+}
+
+__device__ __forceinline__ float2 ldcg2(const float2* p) { return __ldcg(p); }
+__device__ __forceinline__ double2 dmulc(double2 a, double2 w) {      // a * conj(w)
+  return make_double2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y);
+}
+
+// ------------------------------------------------------------------------------------------------
+// plane_unit: one field component on one xy-plane (k_plane_fast of solve_fast.cuh without the boundary
+// source, which the z-line phase has already added), for a GROUP of N*N/(2E) threads of the CTA.
+// ------------------------------------------------------------------------------------------------
+template <int N, int E, bool EMIT>
+__device__ __forceinline__ void plane_unit(const GeomDev& g, int nz, int z, int comp, const float2* __restrict__ src, float2* P,
+                                           float2* Q, const float* s_sdt, const float* s_kx, int tid, int bar_id, int slot) {
+  using C = PlaneCfg<N>;
+  constexpr int Y2 = C::Y2, T = N / E, SX = C::SX, SU = C::SU, NT = N * N / (2 * E);
+  const int ln = tid % Y2, j = tid / Y2;
+  float2 w[E];
+  load_twiddles<E>(w, g.twx, j);
+  unsigned short sid[E];
+  if (!EMIT) {
+    const unsigned short* st = reinterpret_cast<const unsigned short*>(g.sig_t + (size_t)z * N * N);
+#pragma unroll
+    for (int r = 0; r < E; ++r) sid[r] = __ldg(st + ((j + T * r) * N + 2 * ln) / 2);
+  }
+  const float kyv = __ldg(g.kyf + ln);
+  float2 X[E];
+#pragma unroll
+  for (int r = 0; r < E; ++r) X[r] = ldcg2(src + ((size_t)(j + T * r) * nz + z) * Y2 + ln);
+  if (comp < 2) {
+#pragma unroll
+    for (int r = 0; r < E; ++r) {
+      const float kap = (comp == 0) ? s_kx[j + T * r] : kyv;
+      X[r] = make_float2(kap * X[r].y, -kap * X[r].x);       // -i kappa V~
+    }
+  }
+  // ---- A: inverse transform along x
+  fft_stage1<E, true>(X, w);
+#pragma unroll
+  for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[q];
+  group_sync(bar_id, NT);
+  fft_stage2<E, T, true>(X, j, [&](int q, int jj) { return P[(q * T + jj) * Y2 + ln]; });
+#pragma unroll
+  for (int r = 0; r < E; ++r) Q[ln * SX + j + T * r] = X[r];
+  group_sync(bar_id, NT);
+  // Hermitian completion along y of the two packed real rows (Nyquist = 0)
+#pragma unroll
+  for (int r = 0; r < E; ++r) {
+    if (r < E / 2) {
+      const float4 ab = *reinterpret_cast<const float4*>(&Q[(j + T * r) * SX + 2 * ln]);
+      X[r] = make_float2(ab.x - ab.w, ab.y + ab.z);
+    } else {
+      const int km = N - (j + T * r);
+      if (km == Y2) {
+        X[r] = make_float2(0.f, 0.f);
+      } else {
+        const float4 ab = *reinterpret_cast<const float4*>(&Q[km * SX + 2 * ln]);
+        X[r] = make_float2(ab.x + ab.w, ab.z - ab.y);
+      }
+    }
+  }
+  // ---- B: inverse transform along y -> E at the nodes
+  fft_stage1<E, true>(X, w);
+#pragma unroll
+  for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[q];
+  group_sync(bar_id, NT);
+  fft_stage2<E, T, true>(X, j, [&](int q, int jj) { return P[(q * T + jj) * Y2 + ln]; });
+  if constexpr (EMIT) {
+    float2* st = reinterpret_cast<float2*>(g.stage + (((size_t)slot * 3 + comp) * nz + z) * (size_t)(N * N));
+#pragma unroll
+    for (int r = 0; r < E; ++r) st[((j + T * r) * N + 2 * ln) / 2] = make_float2(X[r].x * g.inv_dt, X[r].y * g.inv_dt);
+    group_sync(bar_id, NT);                     // P is rewritten by the group's next unit
+    return;
+  }
+#pragma unroll
+  for (int r = 0; r < E; ++r) {
+    X[r].x *= s_sdt[sid[r] & 0xff];
+    X[r].y *= s_sdt[sid[r] >> 8];
+  }
+  // ---- C: forward transform along y
+  fft_stage1<E, false>(X, w);
+#pragma unroll
+  for (int q = 0; q < E; ++q) Q[(q * T + j) * Y2 + ln] = X[q];
+  group_sync(bar_id, NT);
+  fft_stage2<E, T, false>(X, j, [&](int q, int jj) { return Q[(q * T + jj) * Y2 + ln]; });
+#pragma unroll
+  for (int r = 0; r < E; ++r) P[(j + T * r) * SU + ln] = X[r];
+  group_sync(bar_id, NT);
+  {
+    const int km = (N - ln) % N;
+    const bool odd = j & 1;
+#pragma unroll
+    for (int r = 0; r < E; ++r) {
+      const int p2 = (j + T * r) >> 1;
+      const float2 zk = P[ln * SU + p2], zm = P[km * SU + p2];
+      X[r] = odd ? make_float2(0.5f * (zk.y + zm.y), 0.5f * (zm.x - zk.x))
+                 : make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
+    }
+  }
+  // ---- D: forward transform along x
+  fft_stage1<E, false>(X, w);
+#pragma unroll
+  for (int q = 0; q < E; ++q) Q[(q * T + j) * Y2 + ln] = X[q];
+  group_sync(bar_id, NT);
+  fft_stage2<E, T, false>(X, j, [&](int q, int jj) { return Q[(q * T + jj) * Y2 + ln]; });
+  {
+    float2* __restrict__ dst = (comp == 0) ? g.m0 : (comp == 1) ? g.m1 : g.m2;
+#pragma unroll
+    for (int r = 0; r < E; ++r) {
+      const int kx = j + T * r;
+      float2 o = X[r];
+      if (comp < 2) {
+        const float kap = (comp == 0) ? s_kx[kx] : kyv;
+        o = make_float2(-kap * o.y, kap * o.x);
+      }
+      dst[((size_t)kx * nz + z) * Y2 + ln] = o;
+    }
+  }
+}
+
+// shared memory of one z-line group.  `red` (partial pad-layer sums, written after the per-mode update) lies over
+// `buf` (exchange buffer of the transforms, dead by then: its last reads precede the barrier before the update).
+template <int NZ, int E, int TYL> struct ZGroupSmem {
+  using C = PencilCfg<NZ, E, TYL>;
+  static constexpr size_t buf = 0;                                                   // float2 [2][E][QS]
+  static constexpr size_t red = 0;                                                   // double2 [LT][TYL][2T]  (aliases buf)
+  static constexpr size_t buf_bytes = (size_t)2 * C::FIELD * sizeof(float2);
+  static constexpr size_t red_bytes = (size_t)kMaxLayers * TYL * 2 * C::T * sizeof(double2);
+  static constexpr size_t kzb = (buf_bytes > red_bytes ? buf_bytes : red_bytes);     // float2 [2][NZ][TYL]
+  static constexpr size_t pls = kzb + (size_t)2 * NZ * TYL * sizeof(float2);         // double2 [kMaxLayers][TYL]
+  static constexpr size_t bytes = pls + (size_t)kMaxLayers * TYL * sizeof(double2);
+};
+
+// ------------------------------------------------------------------------------------------------
+// z_pass_a: forward z DFT of (D~, J~z), per-mode Euler update of the fp64 state, V^_rho, pad-layer
+// potentials of this tile (fp64) and their contribution to V_rho at every pad node (added to acc_pad).
+// Thread mapping of k_pencil2 (solve_fast.cuh): (f, line, j), 2 * TYL * NZ/E threads.
+// ------------------------------------------------------------------------------------------------
+template <int NZ, int E, int TYL, int LT, bool APPLY_J, bool DELTA>
+__device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigned char* gsm, const double* s_kz, const double2* s_twz,
+                                         const double2* s_twx, const double2* s_twy, const int* s_px, const int* s_py, const int* s_pl,
+                                         double* acc_pad, int tid, int bar_id) {
+  using C = PencilCfg<NZ, E, TYL>;
+  using S = ZGroupSmem<NZ, E, TYL>;
+  constexpr int T = C::T, QS = C::QS, FIELD = C::FIELD, HT = C::THREADS, NT = 2 * HT;
+  const GeomDev& g = a.g;
+  const int nx = a.gd.nx, ny = a.gd.ny, y2 = a.gd.y2;
+  const int tiles = y2 / TYL;
+  const int kx = tile / tiles, ky0 = (tile % tiles) * TYL;
+  const int f = tid / HT, th = tid % HT;
+  const int line = th % TYL, j = th / TYL;
+  const int ky = ky0 + line;
+  const int L = g.L;
+  float2* buf = reinterpret_cast<float2*>(gsm + S::buf) + f * FIELD;
+  float2* kzb = reinterpret_cast<float2*>(gsm + S::kzb);
+  double2* red = reinterpret_cast<double2*>(gsm + S::red);
+  double2* pls = reinterpret_cast<double2*>(gsm + S::pls);
+  const size_t slab = (size_t)kx * NZ * y2 + ky;
+
+  if constexpr (APPLY_J) {
+    float2 w[E];
+    load_twiddles<E>(w, g.twz, j);
+    float2 X[E];
+    if (f == 0) {
+      const float2* __restrict__ m0 = g.m0 + slab;
+      const float2* __restrict__ m1 = g.m1 + slab;
+#pragma unroll
+      for (int r = 0; r < E; ++r) {
+        const size_t o = (size_t)(j + T * r) * y2;
+        const float2 p = ldcg2(m0 + o), q = ldcg2(m1 + o);
+        X[r] = make_float2(p.x + q.x, p.y + q.y);      // D~ = i kx J~x + i ky J~y
+      }
+    } else {
+      const float2* __restrict__ m2 = g.m2 + slab;
+#pragma unroll
+      for (int r = 0; r < E; ++r) X[r] = ldcg2(m2 + (size_t)(j + T * r) * y2);
+    }
+    fft_stage1<E, false>(X, w);
+#pragma unroll
+    for (int q = 0; q < E; ++q) buf[q * QS + j * TYL + line] = X[q];
+    group_sync(bar_id, NT);
+    fft_stage2<E, T, false>(X, j, [&](int q, int jj) { return buf[q * QS + jj * TYL + line]; });
+#pragma unroll
+    for (int p = 0; p < E; ++p) kzb[(f * NZ + j + T * p) * TYL + line] = X[p];
+    group_sync(bar_id, NT);
+  }
+  {
+    double2 acc[LT];
+#pragma unroll
+    for (int l = 0; l < LT; ++l) acc[l] = make_double2(0.0, 0.0);
+    const double kxd = g.kxd[kx], kyd = g.kyd[ky];
+    const double kxy2 = kxd * kxd + kyd * kyd;
+    const bool ret_x = (kx != nx / 2);
+    double2* __restrict__ rh = g.rhat + slab;
+    const double2* __restrict__ rp = g.rhat_prev + slab;
+#pragma unroll
+    for (int i = 0; i < E / 2; ++i) {
+      const int kz = j + T * (2 * i + f);
+      const size_t o = (size_t)kz * y2;
+      const bool ret = ret_x && (kz != NZ / 2);
+      const double kzd = s_kz[kz];
+      double2 rr = rh[o];
+      if constexpr (APPLY_J) {
+        const float2 D = kzb[kz * TYL + line], J = kzb[(NZ + kz) * TYL + line];
+        const float kzf = (float)kzd;
+        rr.x -= (double)(D.x - kzf * J.y);
+        rr.y -= (double)(D.y + kzf * J.x);
+        if (!ret) rr = make_double2(0.0, 0.0);
+        rh[o] = rr;
+      }
+      double2 src = rr;
+      if constexpr (DELTA) {
+        const double2 p = rp[o];
+        src.x -= p.x; src.y -= p.y;
+      }
+      const double k2 = kxy2 + kzd * kzd;
+      const double gg = (ret && k2 > 0.0) ? a.gd.inv_n * fast_rcp(k2) : 0.0;
+      const double2 v = make_double2(src.x * gg, src.y * gg);
+#pragma unroll
+      for (int l = 0; l < LT; ++l) {
+        if (l < L) {
+          const double2 p = dmulc(v, s_twz[(kz * g.layers[l]) & (NZ - 1)]);      // v e^{+i kz z_l}
+          acc[l].x += p.x; acc[l].y += p.y;
+        }
+      }
+    }
+#pragma unroll
+    for (int l = 0; l < LT; ++l)
+      if (l < L) red[(l * TYL + line) * (2 * T) + f * T + j] = acc[l];
+  }
+  group_sync(bar_id, NT);
+  for (int i = tid; i < L * TYL; i += NT) {       // V~_rho(kx, z_l, ky) in fp64, fixed summation order
+    double2 s = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < 2 * T; ++k) { const double2 p = red[i * (2 * T) + k]; s.x += p.x; s.y += p.y; }
+    const int ln = i % TYL;
+    const double wgt = (ky0 + ln == 0) ? 1.0 : 2.0;          // Hermitian half spectrum along y
+    pls[i] = make_double2(wgt * s.x, wgt * s.y);
+  }
+  group_sync(bar_id, NT);
+  // contribution of this tile to V_rho at every pad node: Re( e^{+i kx x_b} sum_ky pl[l_b][ky] e^{+i ky y_b} )
+  for (int b = tid; b < g.B; b += NT) {
+    const int l = s_pl[b], y = s_py[b];
+    double2 u = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int ln = 0; ln < TYL; ++ln) {
+      const double2 p = dmulc(pls[l * TYL + ln], s_twy[((ky0 + ln) * y) & (ny - 1)]);
+      u.x += p.x; u.y += p.y;
+    }
+    const double2 wx = s_twx[(kx * s_px[b]) & (nx - 1)];
+    acc_pad[b] += u.x * wx.x + u.y * wx.y;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// z_pass_b: V^ = (src + sum_l S_l e^{-i kz z_l}) / |kappa|^2 with S_l(kx, ky) = sum_{b in l} Q'_b e^{-i(kx x_b + ky y_b)}
+// the spectrum of the boundary point charges (a4), -i kz V^, inverse z DFTs -> (oV, oE).
+// ------------------------------------------------------------------------------------------------
+template <int NZ, int E, int TYL, int LT, bool DELTA>
+__device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigned char* gsm, const double* s_kz, const double2* s_twz,
+                                         const double2* s_twx, const double2* s_twy, const int* s_px, const int* s_py,
+                                         const double* s_q, float2* __restrict__ oV, float2* __restrict__ oE, int tid, int bar_id) {
+  using C = PencilCfg<NZ, E, TYL>;
+  using S = ZGroupSmem<NZ, E, TYL>;
+  constexpr int T = C::T, QS = C::QS, FIELD = C::FIELD, HT = C::THREADS, NT = 2 * HT;
+  const GeomDev& g = a.g;
+  const int nx = a.gd.nx, ny = a.gd.ny, y2 = a.gd.y2;
+  const int tiles = y2 / TYL;
+  const int kx = tile / tiles, ky0 = (tile % tiles) * TYL;
+  const int f = tid / HT, th = tid % HT;
+  const int line = th % TYL, j = th / TYL;
+  const int ky = ky0 + line;
+  const int L = g.L;
+  float2* buf = reinterpret_cast<float2*>(gsm + S::buf) + f * FIELD;
+  float2* kzb = reinterpret_cast<float2*>(gsm + S::kzb);
+  double2* pls = reinterpret_cast<double2*>(gsm + S::pls);       // reused: S_l(kx, ky0 + line)
+  const size_t slab = (size_t)kx * NZ * y2 + ky;
+  const int warp = tid >> 5, lane = tid & 31;
+  // one warp per (layer, line): lanes stride over the pads of the layer, fixed shuffle tree
+  for (int o = warp; o < L * TYL; o += NT / 32) {
+    const int l = o / TYL, ln = o - l * TYL;
+    double2 s = make_double2(0.0, 0.0);
+    for (int b = a.lpoff[l] + lane; b < a.lpoff[l + 1]; b += 32) {
+      const double2 c = dmul(s_twx[(kx * s_px[b]) & (nx - 1)], s_twy[((ky0 + ln) * s_py[b]) & (ny - 1)]);
+      const double q = s_q[b];
+      s.x += q * c.x; s.y += q * c.y;
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) { s.x += __shfl_xor_sync(0xffffffffu, s.x, d); s.y += __shfl_xor_sync(0xffffffffu, s.y, d); }
+    if (lane == 0) pls[o] = s;
+  }
+  group_sync(bar_id, NT);
+  {
+    const double kxd = g.kxd[kx], kyd = g.kyd[ky];
+    const double kxy2 = kxd * kxd + kyd * kyd;
+    const bool ret_x = (kx != nx / 2);
+    const double2* __restrict__ rh = g.rhat + slab;
+    double2* __restrict__ rp = g.rhat_prev + slab;
+#pragma unroll
+    for (int i = 0; i < E / 2; ++i) {
+      const int kz = j + T * (2 * i + f);
+      const size_t o = (size_t)kz * y2;
+      const bool ret = ret_x && (kz != NZ / 2);
+      const double kzd = s_kz[kz];
+      const double2 rr = rh[o];
+      double2 src = rr;
+      if constexpr (DELTA) {
+        const double2 p = rp[o];
+        src.x -= p.x; src.y -= p.y;
+        rp[o] = rr;
+      }
+#pragma unroll
+      for (int l = 0; l < LT; ++l) {
+        if (l < L) {
+          const double2 p = dmul(pls[l * TYL + line], s_twz[(kz * g.layers[l]) & (NZ - 1)]);   // S_l e^{-i kz z_l}
+          src.x += p.x; src.y += p.y;
+        }
+      }
+      const double k2 = kxy2 + kzd * kzd;
+      const double gg = (ret && k2 > 0.0) ? a.gd.inv_n * fast_rcp(k2) : 0.0;
+      const double2 v = make_double2(src.x * gg, src.y * gg);
+      kzb[kz * TYL + line] = make_float2((float)v.x, (float)v.y);
+      kzb[(NZ + kz) * TYL + line] = make_float2((float)(kzd * v.y), (float)(-kzd * v.x));   // -i kz V^
+    }
+  }
+  group_sync(bar_id, NT);
+  float2 w[E];
+  load_twiddles<E>(w, g.twz, j);
+  float2 X[E];
+#pragma unroll
+  for (int r = 0; r < E; ++r) X[r] = kzb[(f * NZ + j + T * r) * TYL + line];
+  fft_stage1<E, true>(X, w);
+#pragma unroll
+  for (int q = 0; q < E; ++q) buf[q * QS + j * TYL + line] = X[q];
+  group_sync(bar_id, NT);
+  fft_stage2<E, T, true>(X, j, [&](int q, int jj) { return buf[q * QS + jj * TYL + line]; });
+  {
+    float2* __restrict__ out = (f == 0 ? oV : oE) + slab;
+#pragma unroll
+    for (int r = 0; r < E; ++r) out[(size_t)(j + T * r) * y2] = X[r];
+  }
+  group_sync(bar_id, NT);      // buf / kzb / pls are rewritten by the group's next tile
+}
+
+// ------------------------------------------------------------------------------------------------
+// The kernel.  grid = n_z_cta + n_b_cta CTAs of kPersistThreads threads (cooperative launch: all resident).
+// Dynamic shared memory: [tables][phase region][Ainv slice (B CTAs)].
+// ------------------------------------------------------------------------------------------------
+template <int N, int EP, int NZ, int EZ, int TYL> struct PersistCfg {
+  static constexpr int PT = N * N / (2 * EP);                       // threads of a plane group
+  static constexpr int ZT = 2 * PencilCfg<NZ, EZ, TYL>::THREADS;    // threads of a z-line group
+  static constexpr int PG = kPersistThreads / PT, ZG = kPersistThreads / ZT;
+  static_assert(PG >= 1 && ZG >= 1 && PG <= 8 && ZG <= 8, "group sizes");
+  static constexpr size_t p_bytes = (size_t)PG * 2 * PlaneCfg<N>::BUF * sizeof(float2);
+  static constexpr size_t z_bytes = (size_t)ZG * ZGroupSmem<NZ, EZ, TYL>::bytes;
+  static constexpr size_t t_bytes = (size_t)kStageSlots * 3 * N * sizeof(float);
+  static constexpr size_t phase_bytes = (p_bytes > z_bytes ? p_bytes : z_bytes) > t_bytes ? (p_bytes > z_bytes ? p_bytes : z_bytes) : t_bytes;
+};
+
+struct PersistSmem {        // byte offsets of the table section (host and device agree through this function)
+  size_t kz, twz, twx, twy, px, py, pl, vpad, q, rhs, acc, sdt, kxf, phase, total_tables;
+};
+__host__ __device__ inline PersistSmem persist_smem(int nx, int ny, int nz, int B, int zg) {
+  PersistSmem s;
+  size_t p = 0;
+  auto take = [&](size_t b) { size_t at = p; p = (p + b + 15) / 16 * 16; return at; };
+  s.kz = take((size_t)nz * 8); s.twz = take((size_t)nz * 16); s.twx = take((size_t)nx * 16); s.twy = take((size_t)ny * 16);
+  s.px = take((size_t)B * 4); s.py = take((size_t)B * 4); s.pl = take((size_t)B * 4);
+  s.vpad = take((size_t)B * 8); s.q = take((size_t)B * 8); s.rhs = take((size_t)B * 8);
+  s.acc = take((size_t)zg * B * 8);
+  s.sdt = take(256 * 4); s.kxf = take((size_t)nx * 4);
+  s.phase = p; s.total_tables = p;
+  return s;
+}
+
+template <int N, int EP, int NZ, int EZ, int TYL, int LT>
+__global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_constant__ PersistArgs a) {
+  using CF = PersistCfg<N, EP, NZ, EZ, TYL>;
+  constexpr int PT = CF::PT, ZT = CF::ZT, PG = CF::PG, ZG = CF::ZG;
+  const GeomDev& g = a.g;
+  PersistCtl* ctl = a.ctl;
+  if (*reinterpret_cast<volatile int*>(&ctl->abort)) return;
+  const int tid = threadIdx.x, cta = blockIdx.x, n_cta = gridDim.x;
+  const int B = g.B, Bs = g.Bs, L = g.L;
+  const int nx = N, ny = N, y2 = N / 2, nz = NZ;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  const PersistSmem so = persist_smem(nx, ny, nz, B, ZG);
+  double* s_kz = reinterpret_cast<double*>(smraw + so.kz);
+  double2* s_twz = reinterpret_cast<double2*>(smraw + so.twz);
+  double2* s_twx = reinterpret_cast<double2*>(smraw + so.twx);
+  double2* s_twy = reinterpret_cast<double2*>(smraw + so.twy);
+  int* s_px = reinterpret_cast<int*>(smraw + so.px);
+  int* s_py = reinterpret_cast<int*>(smraw + so.py);
+  int* s_pl = reinterpret_cast<int*>(smraw + so.pl);
+  double* s_vpad = reinterpret_cast<double*>(smraw + so.vpad);
+  double* s_q = reinterpret_cast<double*>(smraw + so.q);
+  double* s_rhs = reinterpret_cast<double*>(smraw + so.rhs);
+  double* s_acc = reinterpret_cast<double*>(smraw + so.acc);
+  float* s_sdt = reinterpret_cast<float*>(smraw + so.sdt);
+  float* s_kxf = reinterpret_cast<float*>(smraw + so.kxf);
+  unsigned char* phase = smraw + so.phase;
+  double* s_ainv = reinterpret_cast<double*>(smraw + a.smem_ainv_off);
+  __shared__ int s_ok;
+
+  const bool is_z = cta < a.n_z_cta;
+  const int brank = cta - a.n_z_cta;                       // rank among the B CTAs (>= 0 for them)
+  const int rows_per = (B + a.n_b_cta - 1) / a.n_b_cta;
+  const int r0 = is_z ? 0 : min(B, brank * rows_per), r1 = is_z ? 0 : min(B, r0 + rows_per);
+
+  for (int i = tid; i < nz; i += kPersistThreads) { s_kz[i] = g.kzd[i]; s_twz[i] = g.twzd[i]; }
+  for (int i = tid; i < nx; i += kPersistThreads) { s_twx[i] = g.twxd[i]; s_kxf[i] = g.kxf[i]; }
+  for (int i = tid; i < ny; i += kPersistThreads) s_twy[i] = g.twyd[i];
+  for (int i = tid; i < 256; i += kPersistThreads) s_sdt[i] = g.sdt[i];
+  for (int i = tid; i < B; i += kPersistThreads) { s_px[i] = a.pad_x[i]; s_py[i] = g.pad_y[i]; s_pl[i] = a.pad_l[i]; s_vpad[i] = g.pad_pot[i]; }
+  if (!is_z && a.ainv_in_smem)
+    for (int i = tid; i < (r1 - r0) * Bs; i += kPersistThreads) s_ainv[i] = g.ainv[(size_t)r0 * Bs + i];
+  __syncthreads();
+
+  unsigned long long bar_n = a.bar0, epi = a.epi0;
+  auto grid_barrier = [&]() -> bool {
+    cta_signal(&ctl->bar);
+    ++bar_n;
+    return cta_wait(&ctl->bar, bar_n * (unsigned long long)n_cta, &ctl->abort, &s_ok);
+  };
+
+  // ---- phases ---------------------------------------------------------------------------------
+  auto plane_phase = [&](auto emit_tag, const float2* srcV, const float2* srcE, int slot) {
+    constexpr bool EMIT = decltype(emit_tag)::value;
+    const int grp = tid / PT, t = tid % PT;
+    float2* P = reinterpret_cast<float2*>(phase) + (size_t)grp * 2 * PlaneCfg<N>::BUF;
+    float2* Q = P + PlaneCfg<N>::BUF;
+    const int n_units = nz * 3, n_slots = n_cta * PG;
+    for (int u = cta * PG + grp; u < n_units; u += n_slots) {
+      const int z = u / 3, comp = u - 3 * z;
+      plane_unit<N, EP, EMIT>(g, nz, z, comp, comp == 2 ? srcE : srcV, P, Q, s_sdt, s_kxf, t, 1 + grp, slot);
+    }
+  };
+  // z-line phase incl. the boundary adjust; flag = 1: pads at their potentials, 0: homogeneous (increment)
+  auto z_phase = [&](auto apply_tag, auto delta_tag, double flag, float2* oV, float2* oE) -> bool {
+    constexpr bool APPLY_J = decltype(apply_tag)::value;
+    constexpr bool DELTA = decltype(delta_tag)::value;
+    ++epi;
+    const int n_tiles = nx * (y2 / TYL);
+    if (is_z) {
+      const int grp = tid / ZT, t = tid % ZT;
+      unsigned char* gsm = phase + (size_t)grp * ZGroupSmem<NZ, EZ, TYL>::bytes;
+      double* acc = s_acc + (size_t)grp * B;
+      for (int b = t; b < B; b += ZT) acc[b] = 0.0;
+      group_sync(1 + grp, ZT);
+      for (int tile = cta + a.n_z_cta * grp; tile < n_tiles; tile += a.n_z_cta * ZG)
+        z_pass_a<NZ, EZ, TYL, LT, APPLY_J, DELTA>(a, tile, gsm, s_kz, s_twz, s_twx, s_twy, s_px, s_py, s_pl, acc, t, 1 + grp);
+      __syncthreads();
+      for (int b = tid; b < B; b += kPersistThreads) {
+        double s = 0.0;
+#pragma unroll
+        for (int q = 0; q < ZG; ++q) s += s_acc[(size_t)q * B + b];
+        a.part[(size_t)b * a.part_stride + cta] = s;
+      }
+      cta_signal(&ctl->cnt_part);
+      if (!cta_wait(&ctl->cnt_q, epi * (unsigned long long)a.n_b_cta, &ctl->abort, &s_ok)) return false;
+      for (int b = tid; b < B; b += kPersistThreads) s_q[b] = __ldcg(g.q + b);
+      __syncthreads();
+      for (int tile = cta + a.n_z_cta * grp; tile < n_tiles; tile += a.n_z_cta * ZG)
+        z_pass_b<NZ, EZ, TYL, LT, DELTA>(a, tile, gsm, s_kz, s_twz, s_twx, s_twy, s_px, s_py, s_q, oV, oE, t, 1 + grp);
+    } else {
+      // ---- boundary adjust on the B CTAs: rows [r0, r1) --------------------------------------------
+      const int warp = tid >> 5, lane = tid & 31;
+      constexpr int kWarps = kPersistThreads / 32;
+      if (!cta_wait(&ctl->cnt_part, epi * (unsigned long long)a.n_z_cta, &ctl->abort, &s_ok)) return false;
+      for (int b = r0 + warp; b < r1; b += kWarps) {          // rhs_b = flag V_pad - sum_c part[b][c], fixed order
+        const double* __restrict__ row = a.part + (size_t)b * a.part_stride;
+        double s = 0.0;
+        for (int c = lane; c < a.n_z_cta; c += 32) s += __ldcg(row + c);
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+        if (lane == 0) g.rhs[b] = flag * s_vpad[b] - s;
+      }
+      cta_signal(&ctl->cnt_rhs);
+      if (!cta_wait(&ctl->cnt_rhs, epi * (unsigned long long)a.n_b_cta, &ctl->abort, &s_ok)) return false;
+      for (int b = tid; b < B; b += kPersistThreads) s_rhs[b] = __ldcg(g.rhs + b);
+      __syncthreads();
+      for (int row = r0 + warp; row < r1; row += kWarps) {     // Q' = Ainv rhs, one warp per row, fixed order
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+        int jj = lane;
+        if (a.ainv_in_smem) {
+          const double* __restrict__ ar = s_ainv + (size_t)(row - r0) * Bs;
+          for (; jj + 96 < B; jj += 128) {
+            s0 += ar[jj] * s_rhs[jj]; s1 += ar[jj + 32] * s_rhs[jj + 32];
+            s2 += ar[jj + 64] * s_rhs[jj + 64]; s3 += ar[jj + 96] * s_rhs[jj + 96];
+          }
+          for (; jj < B; jj += 32) s0 += ar[jj] * s_rhs[jj];
+        } else {
+          const double* __restrict__ ar = g.ainv + (size_t)row * Bs;
+          for (; jj + 96 < B; jj += 128) {
+            s0 += ar[jj] * s_rhs[jj]; s1 += ar[jj + 32] * s_rhs[jj + 32];
+            s2 += ar[jj + 64] * s_rhs[jj + 64]; s3 += ar[jj + 96] * s_rhs[jj + 96];
+          }
+          for (; jj < B; jj += 32) s0 += ar[jj] * s_rhs[jj];
+        }
+        double s = (s0 + s1) + (s2 + s3);
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
+        if (lane == 0) g.q[row] = s;
+      }
+      cta_signal(&ctl->cnt_q);
+    }
+    return true;
+  };
+  auto transpose_phase = [&](int n) {
+    // staging [slot][comp][z][y][x] -> H[((x*ny+y)*nz+z)*nt + t][comp] for the last cnt output steps (k_transpose<true>)
+    const int cnt = n % kStageSlots + 1, t0 = n - cnt + 1, rows = cnt * 3;
+    float* tile = reinterpret_cast<float*>(phase);
+    const int nt = a.gd.nt;
+    for (int unit = cta; unit < nz * ny; unit += n_cta) {
+      const int z = unit / ny, y = unit - z * ny;
+      for (int t = tid; t < rows * nx; t += kPersistThreads) {
+        const int j = t / nx, x = t - j * nx;
+        tile[t] = __ldcg(g.stage + (((size_t)j * nz + z) * ny + y) * nx + x);
+      }
+      __syncthreads();
+      for (int t = tid; t < rows * nx; t += kPersistThreads) {
+        const int x = t / rows, j = t - x * rows;
+        g.H[((((size_t)x * ny + y) * nz + z) * nt + t0) * 3 + j] = tile[j * nx + x];
+      }
+      __syncthreads();
+    }
+  };
+
+  using TT = std::true_type;
+  using FF = std::false_type;
+  const int n = a.step;
+  const int slot = n % kStageSlots;
+  if (n == 0) {
+    // prompt response: r = 0, pads at their potentials.  The same potential starts the step pipeline.
+    if (!z_phase(FF{}, FF{}, 1.0, g.v0, g.v1)) return;
+    if (!grid_barrier()) return;
+    plane_phase(TT{}, g.v0, g.v1, slot);
+  } else {
+    for (int s = 0; s < a.n_sub; ++s) {
+      plane_phase(FF{}, g.v0, g.v1, 0);
+      if (!grid_barrier()) return;
+      if (!z_phase(TT{}, FF{}, 1.0, g.v0, g.v1)) return;
+      if (!grid_barrier()) return;
+    }
+    // H[n] from the increment of the charge since the previous output step, pads at 0 V
+    if (!z_phase(FF{}, TT{}, 0.0, g.e0, g.e1)) return;
+    if (!grid_barrier()) return;
+    plane_phase(TT{}, g.e0, g.e1, slot);
+  }
+  if ((n + 1) % kStageSlots == 0 || n == a.gd.nt - 1) {
+    if (!grid_barrier()) return;
+    transpose_phase(n);
+  }
+}
+
+// last launch of a persistent solve: a time-out anywhere poisons the table (the call is asynchronous: this is
+// how the caller learns about it)
+__global__ void k_persist_finish(PersistCtl* ctl, float* H) {
+  if (ctl->abort) H[0] = __int_as_float(0x7fc00000);
+}
+
+}  // namespace wt

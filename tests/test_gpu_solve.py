@@ -221,6 +221,8 @@ def test_full_grid_window_matches_the_oracle(name, full_size_oracles):
     d_full = geometry_desc(spec["config"])
     nt = spec["nt"]
     g = wt.wt_make_geometry(d_full)
+    plan = wt.wt_describe_plan(g)
+    assert plan.startswith("persistent" if name in ("cfg1", "cfg2") else "chain: k_plane + k_spectral + k_boundary<1|2|3>"), plan
     (H,) = wt.wt_solve_H([g])
     torch.cuda.synchronize()
     h = H[:, :, :, :nt].contiguous().cpu().numpy()
