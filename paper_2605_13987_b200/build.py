@@ -80,4 +80,6 @@ def build(force=False, verbose=False, defines=()):
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    # --debug: -DWTIDE_DEBUG (clock stamps and kernel-skipping switches for timing experiments; never shipped)
+    print(build(force="--force" in sys.argv or "--debug" in sys.argv, verbose="-v" in sys.argv,
+                defines=("WTIDE_DEBUG",) if "--debug" in sys.argv else ()))

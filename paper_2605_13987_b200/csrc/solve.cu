@@ -93,8 +93,11 @@ Layout make_layout(const wt_geometry* g) {
   o.m0 = take(half * 8); o.m1 = take(half * 8); o.m2 = take(half * 8); o.e0 = take(half * 8); o.e1 = take(half * 8);
   o.pl = take(L * nx * y2 * 16); o.pl_e = take(L * nx * y2 * 16);
   o.rhs = take(B * 8); o.q = take(B * 8); o.qh = take(L * nx * y2 * 8);
-  o.part = take(B * (size_t)kPartStride * 8); o.ctl = take(256);
+  o.part = take(((B + 1) & ~(size_t)1) * 2 * 8); o.ctl = take(256);   // (persistent kernel: int64 pad potentials, control block)
   o.stage = take((size_t)kStageSlots * 3 * N * 4);
+#ifdef WTIDE_DEBUG
+  o.dbg = take(256 * 1024);
+#endif
   o.total = p;
   return o;
 }
@@ -272,6 +275,10 @@ extern "C" int wt_solve_H(wt_geometry* const* geoms, int n_geoms, float* const* 
   wt_set_error("");
   return WT_OK;
 }
+
+#ifdef WTIDE_DEBUG
+extern "C" int64_t wt_debug_stamps_offset(const wt_geometry* g) { return (int64_t)make_layout(g).dbg; }
+#endif
 
 extern "C" int wt_describe_plan(const wt_geometry* g, char* out, size_t out_bytes) {
   if (!wt_valid(g) || !out || out_bytes == 0) { wt_set_error("wt_describe_plan: bad argument"); return WT_EINVAL; }

@@ -17,31 +17,34 @@ constexpr int kMaxPadsPersistent = 1100;     // beyond: the kernel chain (Ainv s
 
 struct Variant {
   const void* fn;
-  int tyl, pg, zg;
-  size_t phase_bytes;
+  int tyl, pg, zg, max_pads;
+  bool res;                 // one tile per z-line group, state resident in shared memory
+  size_t phase_bytes, state_bytes;
 };
 
-template <int N, int EP, int NZ, int EZ, int TYL>
+template <int N, int EP, int NZ, int EZ, int TYL, bool RES>
 Variant variant(int L) {
   using CF = PersistCfg<N, EP, NZ, EZ, TYL>;
   Variant v;
-  v.fn = (L <= 2) ? (const void*)k_persistent<N, EP, NZ, EZ, TYL, 2> : (const void*)k_persistent<N, EP, NZ, EZ, TYL, kMaxLayers>;
-  v.tyl = TYL; v.pg = CF::PG; v.zg = CF::ZG;
+  v.fn = (L <= 2) ? (const void*)k_persistent<N, EP, NZ, EZ, TYL, 2, RES> : (const void*)k_persistent<N, EP, NZ, EZ, TYL, kMaxLayers, RES>;
+  v.tyl = TYL; v.pg = CF::PG; v.zg = CF::ZG; v.res = RES;
+  v.max_pads = ZGroupSmem<NZ, EZ, TYL>::max_pads;
   v.phase_bytes = CF::phase_bytes;
+  v.state_bytes = RES ? CF::state_bytes : 0;
   return v;
 }
 
 bool pick(int nx, int ny, int nz, int L, Variant* v) {
   if (nx != ny) return false;
-  if (nx == 64 && nz == 256) { *v = variant<64, 8, 256, 16, 8>(L); return true; }      // BASELINE configs 1 and 3
-  if (nx == 128 && nz == 256) { *v = variant<128, 16, 256, 16, 8>(L); return true; }   // config 2
-  if (nx == 32 && nz == 32) { *v = variant<32, 8, 32, 8, 16>(L); return true; }        // config 0
+  if (nx == 64 && nz == 256) { *v = variant<64, 8, 256, 16, 8, true>(L); return true; }       // BASELINE configs 1 and 3
+  if (nx == 128 && nz == 256) { *v = variant<128, 16, 256, 16, 8, false>(L); return true; }   // config 2
+  if (nx == 32 && nz == 32) { *v = variant<32, 8, 32, 8, 16, true>(L); return true; }         // config 0
   return false;
 }
 
 struct Sizing {
   int n_sm = 0, n_z = 0, n_b = 0, ainv_in_smem = 0;
-  size_t smem = 0, ainv_off = 0;
+  size_t smem = 0, persist_off = 0;
   bool ok = false;
 };
 
@@ -54,7 +57,7 @@ Sizing size_launch(const wt_geometry* g, int B, const Variant& v) {
   cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
   if (const char* e = std::getenv("WTIDE_PERSIST_SMS")) n_sm = std::min(n_sm, std::max(2, std::atoi(e)));
-  if (!coop || n_sm < 2 || n_sm > kPartStride) return s;
+  if (!coop || n_sm < 2) return s;
   const int nx = g->nx, ny = g->ny, nz = g->nz, y2 = ny / 2;
   const int n_tiles = nx * (y2 / v.tyl);
   const int nb_min = std::max(1, std::min(20, (B + 31) / 32));
@@ -64,15 +67,17 @@ Sizing size_launch(const wt_geometry* g, int B, const Variant& v) {
   const int p_ctas = (nz * 3 + v.pg - 1) / v.pg;
   const int grid = std::min(n_sm, std::max(n_z + nb_min, p_ctas));
   s.n_sm = n_sm; s.n_z = n_z; s.n_b = grid - n_z;
-  const PersistSmem so = persist_smem(nx, ny, nz, B, v.zg);
-  const size_t fixed = so.total_tables + v.phase_bytes;
-  s.ainv_off = (fixed + 15) / 16 * 16;
+  if (B > v.max_pads) return s;
+  if (v.res && (per != 1 || n_z * v.zg < n_tiles)) return s;      // (RES kernels own exactly one tile per group)
+  const PersistSmem so = persist_smem(nx, ny, nz, B, v.res ? 0 : v.zg);
+  s.persist_off = (so.phase + v.phase_bytes + 15) / 16 * 16;
   const int rows_per = (B + s.n_b - 1) / s.n_b, Bs = (B + 1) & ~1;
-  const size_t slice = (size_t)rows_per * Bs * 8;
+  const size_t bvec = (size_t)2 * Bs * 8, slice = (size_t)rows_per * Bs * 8;
   const size_t budget = (size_t)max_smem - 1024;      // (static shared memory of the kernel)
-  if (s.ainv_off > budget) return s;
-  s.ainv_in_smem = (s.ainv_off + slice <= budget && !env_flag("WTIDE_AINV_GLOBAL")) ? 1 : 0;
-  s.smem = s.ainv_in_smem ? s.ainv_off + slice : s.ainv_off;
+  const size_t need_min = s.persist_off + std::max(v.state_bytes, bvec);
+  if (need_min > budget) return s;
+  s.ainv_in_smem = (s.persist_off + bvec + slice <= budget && !env_flag("WTIDE_AINV_GLOBAL")) ? 1 : 0;
+  s.smem = s.persist_off + std::max(v.state_bytes, bvec + (s.ainv_in_smem ? slice : 0));
   s.ok = true;
   return s;
 }
@@ -91,7 +96,8 @@ void persistent_describe(const wt_geometry* g, std::string* out) {
   const Sizing s = size_launch(g, (int)g->pad_pot.size(), v);
   char buf[256];
   std::snprintf(buf, sizeof buf, "persistent: k_persistent<%d,%d> (plane_unit + z_pass_a/b + boundary CTAs), %d z-line + %d boundary CTAs, "
-                "one cooperative launch per output step, Ainv %s", g->nx, g->nz, s.n_z, s.n_b, s.ainv_in_smem ? "in shared memory" : "from L2");
+                "one cooperative launch per output step, state %s, Ainv %s", g->nx, g->nz, s.n_z, s.n_b,
+                v.res ? "in shared memory" : "in L2", s.ainv_in_smem ? "in shared memory" : "from L2");
   *out = buf;
 }
 
@@ -120,13 +126,17 @@ int persistent_solve(GeomHost& gh, GridDev gd, cudaStream_t st, SolveStats* stat
   PersistArgs a = {};
   a.g = gh.dev; a.gd = gd;
   a.ctl = (PersistCtl*)(gh.base + gh.lo.ctl);
-  a.part = (double*)(gh.base + gh.lo.part);
+  a.fix = (long long*)(gh.base + gh.lo.part);
   a.pad_x = (const int*)(gh.base + gh.lo.pad_x);
   a.pad_l = (const int*)(gh.base + gh.lo.pad_l);
   for (int l = 0; l <= kMaxLayers; ++l) a.lpoff[l] = gh.pg->layer_poff[std::min(l, L)];
-  a.n_z_cta = sz.n_z; a.n_b_cta = sz.n_b; a.part_stride = kPartStride;
-  a.ainv_in_smem = sz.ainv_in_smem; a.smem_ainv_off = (unsigned)sz.ainv_off;
+  a.n_z_cta = sz.n_z; a.n_b_cta = sz.n_b;
+  a.ainv_in_smem = sz.ainv_in_smem; a.smem_persist_off = (unsigned)sz.persist_off;
+#ifdef WTIDE_DEBUG
+  a.stamps = env_flag("WTIDE_STAMPS") ? (unsigned long long*)(gh.base + gh.lo.dbg) : nullptr;
+#endif
   CKP(cudaMemsetAsync(a.ctl, 0, sizeof(PersistCtl), st));
+  CKP(cudaMemsetAsync(a.fix, 0, (size_t)2 * gh.dev.Bs * sizeof(long long), st));
   CKP(cudaMemsetAsync(gh.dev.rhat, 0, half * sizeof(double2), st));
   CKP(cudaMemsetAsync(gh.dev.rhat_prev, 0, half * sizeof(double2), st));
 

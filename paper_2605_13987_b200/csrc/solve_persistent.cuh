@@ -9,12 +9,16 @@
 //   -- grid barrier --
 //   z-line phase  Z CTAs own fixed tiles of z-lines (kx, TYL ky):
 //      pass A     forward z DFT; r^ -= D^ + i kz J^z (a7, fp64 state); V^_rho = r^/|kappa|^2 (a2); potentials of
-//                 the pad layers (fp64) and from them this CTA's contribution to V_rho at EVERY pad node (a3)
-//      boundary   B CTAs (the SMs the z-lines leave idle): rhs = V_pad - sum of the contributions;
+//                 the pad layers (fp64) and from them this CTA's contribution to V_rho at EVERY pad node (a3),
+//                 added to a global int64 fixed-point accumulator per pad (integer adds commute: deterministic)
+//      boundary   B CTAs (the SMs the z-lines leave idle): rhs = V_pad - V_rho|_B;
 //                 Q' = Ainv rhs: "adjusted, in magnitude, to enforce the boundary conditions"
-//      pass B     spectrum of the boundary point charges for the CTA's own lines; V^ = (r^ + Q^)/|kappa|^2, i.e. the
-//                 translated fundamental solutions of PAPER.md:97 summed in spectral space, in fp64 (a4);
+//      pass B     spectrum of the boundary point charges for the CTA's own lines; V^ = V^_rho + Q^/|kappa|^2, i.e. the
+//                 translated fundamental solutions of PAPER.md:97 summed in spectral space (a4);
 //                 inverse z DFT of V^ and -i kz V^                                                  -> v0, v1
+//      With one tile per z-line group (BASELINE configs 0, 1, 3) the fp64 state of the tile lives in shared memory and
+//      its 1/|kappa|^2 factors in registers for the whole launch, and V^_rho waits in shared memory for the charges
+//      (RES); otherwise (config 2) the state stays in global memory and pass B forms V^ from it again.
 //   -- grid barrier --
 // and every n_sub substeps the same phases run on the increment r^ - r^_prev with the pads at 0 V and write
 // H[n] = E/dt (a8) into the staging buffer, which a last phase transposes into the time-innermost table.
@@ -40,16 +44,19 @@ struct PersistArgs {
   GeomDev g;
   GridDev gd;
   PersistCtl* ctl;
-  double* part;                     // [B][part_stride]: contribution of Z CTA c to V_rho at pad b
+  long long* fix;                   // [2][Bs]: V_rho at the pads as int64 fixed point (2^42), double buffered by episode parity
   const int* pad_x;                 // [B] group order
   const int* pad_l;                 // [B] layer index of the pad
   int lpoff[kMaxLayers + 1];        // pads of layer l = [lpoff[l], lpoff[l+1])
-  int n_z_cta, n_b_cta, part_stride;
+  int n_z_cta, n_b_cta;
   int ainv_in_smem;                 // the B CTA's rows of Ainv live in shared memory for the whole launch
-  unsigned smem_ainv_off;           // byte offset of that slice in the dynamic shared memory
+  unsigned smem_persist_off;        // byte offset of the persistent region in the dynamic shared memory
   int step;                         // index n of the output step this launch produces
   int n_sub;                        // Euler substeps before the emit (0 for n = 0)
   unsigned long long bar0, epi0;    // grid barriers / boundary episodes completed by earlier launches
+#ifdef WTIDE_DEBUG
+  unsigned long long* stamps;       // [n_cta][64] globaltimer stamps of thread 0 during output step 2 (timing experiments)
+#endif
 };
 
 constexpr long long kSpinLimit = 4000000000LL;     // cycles (about two seconds)
@@ -86,6 +93,13 @@ __device__ __forceinline__ bool cta_wait(const unsigned long long* ctr, unsigned
   return ok;
 }
 
+#ifdef WTIDE_DEBUG
+// fine stamps of thread 0 (group 0) inside the z passes: slots 32.. of the CTA's row, substep 1 of output step 2 only
+__shared__ int g_fine_on;
+#define FSTAMP(k) do { if (a.stamps && a.step == 2 && threadIdx.x == 0 && g_fine_on) { unsigned long long t_; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t_)); a.stamps[(size_t)blockIdx.x * 64 + 32 + (k)] = t_; } } while (0)
+#else
+#define FSTAMP(k) do { } while (0)
+#endif
 __device__ __forceinline__ float2 ldcg2(const float2* p) { return __ldcg(p); }
 __device__ __forceinline__ double2 dmulc(double2 a, double2 w) {      // a * conj(w)
   return make_double2(a.x * w.x + a.y * w.y, a.y * w.x - a.x * w.y);
@@ -204,28 +218,35 @@ __device__ __forceinline__ void plane_unit(const GeomDev& g, int nz, int z, int 
   }
 }
 
-// shared memory of one z-line group.  `red` (partial pad-layer sums, written after the per-mode update) lies over
-// `buf` (exchange buffer of the transforms, dead by then: its last reads precede the barrier before the update).
+// shared memory of one z-line group (transient part).  `red` (partial pad-layer sums, written after the per-mode
+// update), `accp` (pad contributions, RES mode) and `cs` (charges times e^{-i kx x}, pass B) lie over `buf`
+// (exchange buffer of the transforms), which is dead whenever they are live.
 template <int NZ, int E, int TYL> struct ZGroupSmem {
   using C = PencilCfg<NZ, E, TYL>;
   static constexpr size_t buf = 0;                                                   // float2 [2][E][QS]
-  static constexpr size_t red = 0;                                                   // double2 [LT][TYL][2T]  (aliases buf)
   static constexpr size_t buf_bytes = (size_t)2 * C::FIELD * sizeof(float2);
   static constexpr size_t red_bytes = (size_t)kMaxLayers * TYL * 2 * C::T * sizeof(double2);
   static constexpr size_t kzb = (buf_bytes > red_bytes ? buf_bytes : red_bytes);     // float2 [2][NZ][TYL]
   static constexpr size_t pls = kzb + (size_t)2 * NZ * TYL * sizeof(float2);         // double2 [kMaxLayers][TYL]
   static constexpr size_t bytes = pls + (size_t)kMaxLayers * TYL * sizeof(double2);
+  static constexpr size_t state_bytes = (size_t)NZ * TYL * sizeof(double2);          // RES: the tile's fp64 charge spectrum
+  static constexpr int max_pads = (int)(kzb / 16);                                    // cs[B] double2 must fit over buf
 };
 
+constexpr double kFixScale = 4398046511104.0;            // 2^42: pad potentials are accumulated as int64 fixed point
+constexpr double kFixInv = 1.0 / 4398046511104.0;        // (integer adds commute: the sum over the CTAs is order independent)
+
 // ------------------------------------------------------------------------------------------------
-// z_pass_a: forward z DFT of (D~, J~z), per-mode Euler update of the fp64 state, V^_rho, pad-layer
-// potentials of this tile (fp64) and their contribution to V_rho at every pad node (added to acc_pad).
+// z_pass_a: forward z DFT of (D~, J~z), per-mode Euler update of the fp64 state, V^_rho, pad-layer potentials of
+// this tile (fp64) and their contribution to V_rho at every pad node (added to acc_pad).
 // Thread mapping of k_pencil2 (solve_fast.cuh): (f, line, j), 2 * TYL * NZ/E threads.
+//   RES   the group owns this one tile for the whole launch: its state lives in shared memory (rsm), the inverse
+//         Green factors gg in registers, and V^_rho stays in kzb for z_pass_b
 // ------------------------------------------------------------------------------------------------
-template <int NZ, int E, int TYL, int LT, bool APPLY_J, bool DELTA>
-__device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigned char* gsm, const double* s_kz, const double2* s_twz,
-                                         const double2* s_twx, const double2* s_twy, const int* s_px, const int* s_py, const int* s_pl,
-                                         double* acc_pad, int tid, int bar_id) {
+template <int NZ, int E, int TYL, int LT, bool RES, bool APPLY_J, bool DELTA>
+__device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigned char* gsm, double2* rsm, const double (&gg)[E / 2],
+                                         const double* s_kz, const double2* s_twz, const double2* s_twx, const double2* s_twy,
+                                         const int* s_px, const int* s_py, const int* s_pl, double* acc_pad, int tid, int bar_id) {
   using C = PencilCfg<NZ, E, TYL>;
   using S = ZGroupSmem<NZ, E, TYL>;
   constexpr int T = C::T, QS = C::QS, FIELD = C::FIELD, HT = C::THREADS, NT = 2 * HT;
@@ -239,10 +260,11 @@ __device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigne
   const int L = g.L;
   float2* buf = reinterpret_cast<float2*>(gsm + S::buf) + f * FIELD;
   float2* kzb = reinterpret_cast<float2*>(gsm + S::kzb);
-  double2* red = reinterpret_cast<double2*>(gsm + S::red);
+  double2* red = reinterpret_cast<double2*>(gsm + S::buf);
   double2* pls = reinterpret_cast<double2*>(gsm + S::pls);
   const size_t slab = (size_t)kx * NZ * y2 + ky;
 
+  FSTAMP(0);
   if constexpr (APPLY_J) {
     float2 w[E];
     load_twiddles<E>(w, g.twz, j);
@@ -261,14 +283,17 @@ __device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigne
 #pragma unroll
       for (int r = 0; r < E; ++r) X[r] = ldcg2(m2 + (size_t)(j + T * r) * y2);
     }
+    FSTAMP(1);
     fft_stage1<E, false>(X, w);
 #pragma unroll
     for (int q = 0; q < E; ++q) buf[q * QS + j * TYL + line] = X[q];
     group_sync(bar_id, NT);
+    FSTAMP(2);
     fft_stage2<E, T, false>(X, j, [&](int q, int jj) { return buf[q * QS + jj * TYL + line]; });
 #pragma unroll
     for (int p = 0; p < E; ++p) kzb[(f * NZ + j + T * p) * TYL + line] = X[p];
     group_sync(bar_id, NT);
+    FSTAMP(3);
   }
   {
     double2 acc[LT];
@@ -278,30 +303,40 @@ __device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigne
     const double kxy2 = kxd * kxd + kyd * kyd;
     const bool ret_x = (kx != nx / 2);
     double2* __restrict__ rh = g.rhat + slab;
-    const double2* __restrict__ rp = g.rhat_prev + slab;
+    double2* __restrict__ rp = g.rhat_prev + slab;
 #pragma unroll
     for (int i = 0; i < E / 2; ++i) {
       const int kz = j + T * (2 * i + f);
       const size_t o = (size_t)kz * y2;
       const bool ret = ret_x && (kz != NZ / 2);
       const double kzd = s_kz[kz];
-      double2 rr = rh[o];
+      double2 rr = RES ? rsm[kz * TYL + line] : rh[o];
       if constexpr (APPLY_J) {
         const float2 D = kzb[kz * TYL + line], J = kzb[(NZ + kz) * TYL + line];
         const float kzf = (float)kzd;
         rr.x -= (double)(D.x - kzf * J.y);
         rr.y -= (double)(D.y + kzf * J.x);
         if (!ret) rr = make_double2(0.0, 0.0);
-        rh[o] = rr;
+        if (RES) rsm[kz * TYL + line] = rr; else rh[o] = rr;
       }
       double2 src = rr;
       if constexpr (DELTA) {
         const double2 p = rp[o];
         src.x -= p.x; src.y -= p.y;
+        if (RES) rp[o] = rr;                   // (two-pass mode: z_pass_b reads the old value once more and then writes)
       }
-      const double k2 = kxy2 + kzd * kzd;
-      const double gg = (ret && k2 > 0.0) ? a.gd.inv_n * fast_rcp(k2) : 0.0;
-      const double2 v = make_double2(src.x * gg, src.y * gg);
+      double ggi;
+      if constexpr (RES) {
+        ggi = gg[i];
+      } else {
+        const double k2 = kxy2 + kzd * kzd;
+        ggi = (ret && k2 > 0.0) ? a.gd.inv_n * fast_rcp(k2) : 0.0;
+      }
+      const double2 v = make_double2(src.x * ggi, src.y * ggi);
+      if constexpr (RES) {                     // V^_rho and -i kz V^_rho wait in kzb for the boundary charges
+        kzb[kz * TYL + line] = make_float2((float)v.x, (float)v.y);
+        kzb[(NZ + kz) * TYL + line] = make_float2((float)(kzd * v.y), (float)(-kzd * v.x));
+      }
 #pragma unroll
       for (int l = 0; l < LT; ++l) {
         if (l < L) {
@@ -315,37 +350,50 @@ __device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigne
       if (l < L) red[(l * TYL + line) * (2 * T) + f * T + j] = acc[l];
   }
   group_sync(bar_id, NT);
-  for (int i = tid; i < L * TYL; i += NT) {       // V~_rho(kx, z_l, ky) in fp64, fixed summation order
+  FSTAMP(4);
+  // V~_rho(kx, z_l, ky) in fp64: 16 lanes per sum, fixed order (two terms per lane, then a shuffle tree)
+  for (int i0 = 0; i0 < L * TYL; i0 += NT / 16) {
+    const int i = i0 + tid / 16, sub = tid & 15;
     double2 s = make_double2(0.0, 0.0);
+    if (i < L * TYL) {
+      for (int k = sub; k < 2 * T; k += 16) { const double2 p = red[i * (2 * T) + k]; s.x += p.x; s.y += p.y; }
+    }
 #pragma unroll
-    for (int k = 0; k < 2 * T; ++k) { const double2 p = red[i * (2 * T) + k]; s.x += p.x; s.y += p.y; }
-    const int ln = i % TYL;
-    const double wgt = (ky0 + ln == 0) ? 1.0 : 2.0;          // Hermitian half spectrum along y
-    pls[i] = make_double2(wgt * s.x, wgt * s.y);
+    for (int d = 8; d > 0; d >>= 1) { s.x += __shfl_xor_sync(0xffffffffu, s.x, d); s.y += __shfl_xor_sync(0xffffffffu, s.y, d); }
+    if (i < L * TYL && sub == 0) {
+      const double wgt = (ky0 + i % TYL == 0) ? 1.0 : 2.0;          // Hermitian half spectrum along y
+      pls[i] = make_double2(wgt * s.x, wgt * s.y);
+    }
   }
   group_sync(bar_id, NT);
+  FSTAMP(5);
   // contribution of this tile to V_rho at every pad node: Re( e^{+i kx x_b} sum_ky pl[l_b][ky] e^{+i ky y_b} )
   for (int b = tid; b < g.B; b += NT) {
     const int l = s_pl[b], y = s_py[b];
-    double2 u = make_double2(0.0, 0.0);
+    double2 u0 = make_double2(0.0, 0.0), u1 = make_double2(0.0, 0.0);
 #pragma unroll
-    for (int ln = 0; ln < TYL; ++ln) {
-      const double2 p = dmulc(pls[l * TYL + ln], s_twy[((ky0 + ln) * y) & (ny - 1)]);
-      u.x += p.x; u.y += p.y;
+    for (int ln = 0; ln < TYL; ln += 2) {
+      const double2 p0 = dmulc(pls[l * TYL + ln], s_twy[((ky0 + ln) * y) & (ny - 1)]);
+      const double2 p1 = dmulc(pls[l * TYL + ln + 1], s_twy[((ky0 + ln + 1) * y) & (ny - 1)]);
+      u0.x += p0.x; u0.y += p0.y; u1.x += p1.x; u1.y += p1.y;
     }
     const double2 wx = s_twx[(kx * s_px[b]) & (nx - 1)];
-    acc_pad[b] += u.x * wx.x + u.y * wx.y;
+    const double c = (u0.x + u1.x) * wx.x + (u0.y + u1.y) * wx.y;
+    if (RES) acc_pad[b] = c; else acc_pad[b] += c;
   }
+  FSTAMP(6);
 }
 
 // ------------------------------------------------------------------------------------------------
-// z_pass_b: V^ = (src + sum_l S_l e^{-i kz z_l}) / |kappa|^2 with S_l(kx, ky) = sum_{b in l} Q'_b e^{-i(kx x_b + ky y_b)}
-// the spectrum of the boundary point charges (a4), -i kz V^, inverse z DFTs -> (oV, oE).
+// z_pass_b: V^ = V^_rho + (sum_l S_l e^{-i kz z_l}) / |kappa|^2 with S_l(kx, ky) = sum_{b in l} Q'_b e^{-i(kx x_b + ky y_b)}
+// the spectrum of the boundary point charges (a4: the translated fundamental solutions of PAPER.md:97 summed in
+// spectral space), -i kz V^, inverse z DFTs -> (oV, oE).  RES: V^_rho waits in kzb (fp32) and the source is added in
+// fp32; otherwise V^ is formed again from the fp64 state with the source added in fp64.
 // ------------------------------------------------------------------------------------------------
-template <int NZ, int E, int TYL, int LT, bool DELTA>
-__device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigned char* gsm, const double* s_kz, const double2* s_twz,
-                                         const double2* s_twx, const double2* s_twy, const int* s_px, const int* s_py,
-                                         const double* s_q, float2* __restrict__ oV, float2* __restrict__ oE, int tid, int bar_id) {
+template <int NZ, int E, int TYL, int LT, bool RES, bool DELTA>
+__device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigned char* gsm, const double (&gg)[E / 2], const double* s_kz,
+                                         const double2* s_twz, const double2* s_twx, const double2* s_twy, const int* s_px, const int* s_py,
+                                         float2* __restrict__ oV, float2* __restrict__ oE, int tid, int bar_id) {
   using C = PencilCfg<NZ, E, TYL>;
   using S = ZGroupSmem<NZ, E, TYL>;
   constexpr int T = C::T, QS = C::QS, FIELD = C::FIELD, HT = C::THREADS, NT = 2 * HT;
@@ -356,27 +404,62 @@ __device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigne
   const int f = tid / HT, th = tid % HT;
   const int line = th % TYL, j = th / TYL;
   const int ky = ky0 + line;
-  const int L = g.L;
+  const int L = g.L, B = g.B;
   float2* buf = reinterpret_cast<float2*>(gsm + S::buf) + f * FIELD;
   float2* kzb = reinterpret_cast<float2*>(gsm + S::kzb);
+  double2* cs = reinterpret_cast<double2*>(gsm + S::buf);        // [B] Q'_b e^{-i kx x_b}
   double2* pls = reinterpret_cast<double2*>(gsm + S::pls);       // reused: S_l(kx, ky0 + line)
   const size_t slab = (size_t)kx * NZ * y2 + ky;
-  const int warp = tid >> 5, lane = tid & 31;
-  // one warp per (layer, line): lanes stride over the pads of the layer, fixed shuffle tree
-  for (int o = warp; o < L * TYL; o += NT / 32) {
-    const int l = o / TYL, ln = o - l * TYL;
-    double2 s = make_double2(0.0, 0.0);
-    for (int b = a.lpoff[l] + lane; b < a.lpoff[l + 1]; b += 32) {
-      const double2 c = dmul(s_twx[(kx * s_px[b]) & (nx - 1)], s_twy[((ky0 + ln) * s_py[b]) & (ny - 1)]);
-      const double q = s_q[b];
-      s.x += q * c.x; s.y += q * c.y;
-    }
-#pragma unroll
-    for (int d = 16; d > 0; d >>= 1) { s.x += __shfl_xor_sync(0xffffffffu, s.x, d); s.y += __shfl_xor_sync(0xffffffffu, s.y, d); }
-    if (lane == 0) pls[o] = s;
+  FSTAMP(8);
+  for (int b = tid; b < B; b += NT) {
+    const double q = __ldcg(g.q + b);
+    const double2 wx = s_twx[(kx * s_px[b]) & (nx - 1)];
+    cs[b] = make_double2(q * wx.x, q * wx.y);
   }
   group_sync(bar_id, NT);
-  {
+  // S_l(kx, ky): 16 lanes per sum over the pads of the layer, fixed order
+  for (int i0 = 0; i0 < L * TYL; i0 += NT / 16) {
+    const int i = i0 + tid / 16, sub = tid & 15;
+    double2 s = make_double2(0.0, 0.0);
+    if (i < L * TYL) {
+      const int l = i / TYL, ln = i - l * TYL;
+      for (int b = a.lpoff[l] + sub; b < a.lpoff[l + 1]; b += 16) {
+        const double2 p = dmul(cs[b], s_twy[((ky0 + ln) * s_py[b]) & (ny - 1)]);
+        s.x += p.x; s.y += p.y;
+      }
+    }
+#pragma unroll
+    for (int d = 8; d > 0; d >>= 1) { s.x += __shfl_xor_sync(0xffffffffu, s.x, d); s.y += __shfl_xor_sync(0xffffffffu, s.y, d); }
+    if (i < L * TYL && sub == 0) pls[i] = s;
+  }
+  group_sync(bar_id, NT);
+  FSTAMP(9);
+  if constexpr (RES) {
+    // the source in fp32: kzb += (sum_l S_l e^{-i kz z_l}) gg, and the same times -i kz
+    float2 sl[LT];
+#pragma unroll
+    for (int l = 0; l < LT; ++l) sl[l] = (l < L) ? make_float2((float)pls[l * TYL + line].x, (float)pls[l * TYL + line].y) : make_float2(0.f, 0.f);
+#pragma unroll
+    for (int i = 0; i < E / 2; ++i) {
+      const int kz = j + T * (2 * i + f);
+      float2 src = make_float2(0.f, 0.f);
+#pragma unroll
+      for (int l = 0; l < LT; ++l) {
+        if (l < L) {
+          const double2 wd = s_twz[(kz * g.layers[l]) & (NZ - 1)];
+          const float2 wz = make_float2((float)wd.x, (float)wd.y);
+          src.x += sl[l].x * wz.x - sl[l].y * wz.y; src.y += sl[l].x * wz.y + sl[l].y * wz.x;
+        }
+      }
+      const float gf = (float)gg[i], kzf = (float)s_kz[kz];
+      const float2 v = make_float2(src.x * gf, src.y * gf);
+      float2 c0 = kzb[kz * TYL + line], c1 = kzb[(NZ + kz) * TYL + line];
+      c0.x += v.x; c0.y += v.y;
+      c1.x += kzf * v.y; c1.y -= kzf * v.x;
+      kzb[kz * TYL + line] = c0;
+      kzb[(NZ + kz) * TYL + line] = c1;
+    }
+  } else {
     const double kxd = g.kxd[kx], kyd = g.kyd[ky];
     const double kxy2 = kxd * kxd + kyd * kyd;
     const bool ret_x = (kx != nx / 2);
@@ -403,13 +486,14 @@ __device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigne
         }
       }
       const double k2 = kxy2 + kzd * kzd;
-      const double gg = (ret && k2 > 0.0) ? a.gd.inv_n * fast_rcp(k2) : 0.0;
-      const double2 v = make_double2(src.x * gg, src.y * gg);
+      const double ggi = (ret && k2 > 0.0) ? a.gd.inv_n * fast_rcp(k2) : 0.0;
+      const double2 v = make_double2(src.x * ggi, src.y * ggi);
       kzb[kz * TYL + line] = make_float2((float)v.x, (float)v.y);
       kzb[(NZ + kz) * TYL + line] = make_float2((float)(kzd * v.y), (float)(-kzd * v.x));   // -i kz V^
     }
   }
   group_sync(bar_id, NT);
+  FSTAMP(10);
   float2 w[E];
   load_twiddles<E>(w, g.twz, j);
   float2 X[E];
@@ -419,18 +503,22 @@ __device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigne
 #pragma unroll
   for (int q = 0; q < E; ++q) buf[q * QS + j * TYL + line] = X[q];
   group_sync(bar_id, NT);
+  FSTAMP(11);
   fft_stage2<E, T, true>(X, j, [&](int q, int jj) { return buf[q * QS + jj * TYL + line]; });
   {
     float2* __restrict__ out = (f == 0 ? oV : oE) + slab;
 #pragma unroll
     for (int r = 0; r < E; ++r) out[(size_t)(j + T * r) * y2] = X[r];
   }
+  FSTAMP(12);
   group_sync(bar_id, NT);      // buf / kzb / pls are rewritten by the group's next tile
+  FSTAMP(13);
 }
 
 // ------------------------------------------------------------------------------------------------
 // The kernel.  grid = n_z_cta + n_b_cta CTAs of kPersistThreads threads (cooperative launch: all resident).
-// Dynamic shared memory: [tables][phase region][Ainv slice (B CTAs)].
+// Dynamic shared memory: [tables][transient phase region][persistent region: fp64 state of the CTA's tiles (Z CTAs,
+// RES) | rhs, V_pad and the CTA's rows of Ainv (B CTAs)].
 // ------------------------------------------------------------------------------------------------
 template <int N, int EP, int NZ, int EZ, int TYL> struct PersistCfg {
   static constexpr int PT = N * N / (2 * EP);                       // threads of a plane group
@@ -441,36 +529,39 @@ template <int N, int EP, int NZ, int EZ, int TYL> struct PersistCfg {
   static constexpr size_t z_bytes = (size_t)ZG * ZGroupSmem<NZ, EZ, TYL>::bytes;
   static constexpr size_t t_bytes = (size_t)kStageSlots * 3 * N * sizeof(float);
   static constexpr size_t phase_bytes = (p_bytes > z_bytes ? p_bytes : z_bytes) > t_bytes ? (p_bytes > z_bytes ? p_bytes : z_bytes) : t_bytes;
+  static constexpr size_t state_bytes = (size_t)ZG * ZGroupSmem<NZ, EZ, TYL>::state_bytes;
 };
 
 struct PersistSmem {        // byte offsets of the table section (host and device agree through this function)
-  size_t kz, twz, twx, twy, px, py, pl, vpad, q, rhs, acc, sdt, kxf, phase, total_tables;
+  size_t kz, twz, twx, twy, px, py, pl, acc, sdt, kxf, phase;
 };
-__host__ __device__ inline PersistSmem persist_smem(int nx, int ny, int nz, int B, int zg) {
+// acc_groups: z-line groups that need their own pad accumulators in the table section (0 in RES mode)
+__host__ __device__ inline PersistSmem persist_smem(int nx, int ny, int nz, int B, int acc_groups) {
   PersistSmem s;
   size_t p = 0;
   auto take = [&](size_t b) { size_t at = p; p = (p + b + 15) / 16 * 16; return at; };
   s.kz = take((size_t)nz * 8); s.twz = take((size_t)nz * 16); s.twx = take((size_t)nx * 16); s.twy = take((size_t)ny * 16);
   s.px = take((size_t)B * 4); s.py = take((size_t)B * 4); s.pl = take((size_t)B * 4);
-  s.vpad = take((size_t)B * 8); s.q = take((size_t)B * 8); s.rhs = take((size_t)B * 8);
-  s.acc = take((size_t)zg * B * 8);
+  s.acc = take((size_t)acc_groups * B * 8);
   s.sdt = take(256 * 4); s.kxf = take((size_t)nx * 4);
-  s.phase = p; s.total_tables = p;
+  s.phase = p;
   return s;
 }
 
-template <int N, int EP, int NZ, int EZ, int TYL, int LT>
+template <int N, int EP, int NZ, int EZ, int TYL, int LT, bool RES>
 __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_constant__ PersistArgs a) {
   using CF = PersistCfg<N, EP, NZ, EZ, TYL>;
+  using ZS = ZGroupSmem<NZ, EZ, TYL>;
   constexpr int PT = CF::PT, ZT = CF::ZT, PG = CF::PG, ZG = CF::ZG;
+  constexpr int TZ = NZ / EZ;
   const GeomDev& g = a.g;
   PersistCtl* ctl = a.ctl;
   if (*reinterpret_cast<volatile int*>(&ctl->abort)) return;
   const int tid = threadIdx.x, cta = blockIdx.x, n_cta = gridDim.x;
-  const int B = g.B, Bs = g.Bs, L = g.L;
+  const int B = g.B, Bs = g.Bs;
   const int nx = N, ny = N, y2 = N / 2, nz = NZ;
   extern __shared__ __align__(16) unsigned char smraw[];
-  const PersistSmem so = persist_smem(nx, ny, nz, B, ZG);
+  const PersistSmem so = persist_smem(nx, ny, nz, B, RES ? 0 : ZG);
   double* s_kz = reinterpret_cast<double*>(smraw + so.kz);
   double2* s_twz = reinterpret_cast<double2*>(smraw + so.twz);
   double2* s_twx = reinterpret_cast<double2*>(smraw + so.twx);
@@ -478,30 +569,72 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
   int* s_px = reinterpret_cast<int*>(smraw + so.px);
   int* s_py = reinterpret_cast<int*>(smraw + so.py);
   int* s_pl = reinterpret_cast<int*>(smraw + so.pl);
-  double* s_vpad = reinterpret_cast<double*>(smraw + so.vpad);
-  double* s_q = reinterpret_cast<double*>(smraw + so.q);
-  double* s_rhs = reinterpret_cast<double*>(smraw + so.rhs);
-  double* s_acc = reinterpret_cast<double*>(smraw + so.acc);
   float* s_sdt = reinterpret_cast<float*>(smraw + so.sdt);
   float* s_kxf = reinterpret_cast<float*>(smraw + so.kxf);
   unsigned char* phase = smraw + so.phase;
-  double* s_ainv = reinterpret_cast<double*>(smraw + a.smem_ainv_off);
+  unsigned char* persist = smraw + a.smem_persist_off;
+  // B CTAs: rhs [Bs], V_pad [Bs], rows of Ainv
+  double* s_rhs = reinterpret_cast<double*>(persist);
+  double* s_vpad = s_rhs + Bs;
+  double* s_ainv = s_vpad + Bs;
   __shared__ int s_ok;
 
   const bool is_z = cta < a.n_z_cta;
   const int brank = cta - a.n_z_cta;                       // rank among the B CTAs (>= 0 for them)
   const int rows_per = (B + a.n_b_cta - 1) / a.n_b_cta;
   const int r0 = is_z ? 0 : min(B, brank * rows_per), r1 = is_z ? 0 : min(B, r0 + rows_per);
+  const int n_tiles = nx * (y2 / TYL);
 
   for (int i = tid; i < nz; i += kPersistThreads) { s_kz[i] = g.kzd[i]; s_twz[i] = g.twzd[i]; }
   for (int i = tid; i < nx; i += kPersistThreads) { s_twx[i] = g.twxd[i]; s_kxf[i] = g.kxf[i]; }
   for (int i = tid; i < ny; i += kPersistThreads) s_twy[i] = g.twyd[i];
   for (int i = tid; i < 256; i += kPersistThreads) s_sdt[i] = g.sdt[i];
-  for (int i = tid; i < B; i += kPersistThreads) { s_px[i] = a.pad_x[i]; s_py[i] = g.pad_y[i]; s_pl[i] = a.pad_l[i]; s_vpad[i] = g.pad_pot[i]; }
-  if (!is_z && a.ainv_in_smem)
-    for (int i = tid; i < (r1 - r0) * Bs; i += kPersistThreads) s_ainv[i] = g.ainv[(size_t)r0 * Bs + i];
+  for (int i = tid; i < B; i += kPersistThreads) { s_px[i] = a.pad_x[i]; s_py[i] = g.pad_y[i]; s_pl[i] = a.pad_l[i]; }
+  if (!is_z) {
+    for (int i = tid; i < B; i += kPersistThreads) s_vpad[i] = g.pad_pot[i];
+    if (a.ainv_in_smem)
+      for (int i = tid; i < (r1 - r0) * Bs; i += kPersistThreads) s_ainv[i] = g.ainv[(size_t)r0 * Bs + i];
+  }
+  // RES: the group's tile, its fp64 state (shared memory) and inverse Green factors (registers) for the whole launch
+  const int zgrp = tid / ZT, zt = tid % ZT;
+  const int my_tile = cta + a.n_z_cta * zgrp;
+  double2* rsm = reinterpret_cast<double2*>(persist + (size_t)zgrp * ZS::state_bytes);
+  double gg[EZ / 2];
+#pragma unroll
+  for (int i = 0; i < EZ / 2; ++i) gg[i] = 0.0;
+  if (RES && is_z && my_tile < n_tiles) {
+    const int tiles = y2 / TYL;
+    const int kx = my_tile / tiles, ky0 = (my_tile % tiles) * TYL;
+    constexpr int HT = ZT / 2;
+    const int f = zt / HT, th = zt % HT, line = th % TYL, j = th / TYL;
+    const double kxd = g.kxd[kx], kyd = g.kyd[ky0 + line];
+#pragma unroll
+    for (int i = 0; i < EZ / 2; ++i) {
+      const int kz = j + TZ * (2 * i + f);
+      const double kzd = g.kzd[kz];
+      const double k2 = kxd * kxd + kyd * kyd + kzd * kzd;
+      gg[i] = (kx != nx / 2 && kz != NZ / 2 && k2 > 0.0) ? a.gd.inv_n / k2 : 0.0;
+    }
+    for (int i = zt; i < NZ * TYL; i += ZT) {
+      const int kz = i / TYL, ln = i - kz * TYL;
+      rsm[i] = g.rhat[((size_t)kx * NZ + kz) * y2 + ky0 + ln];
+    }
+  }
   __syncthreads();
 
+#ifdef WTIDE_DEBUG
+  int n_stamp = 0;
+  auto stamp = [&]() {
+    if (a.stamps && a.step == 2 && tid == 0 && n_stamp < 28) {
+      unsigned long long t;
+      asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t));
+      a.stamps[(size_t)cta * 64 + n_stamp++] = t;
+    }
+  };
+#define PSTAMP() stamp()
+#else
+#define PSTAMP() do { } while (0)
+#endif
   unsigned long long bar_n = a.bar0, epi = a.epi0;
   auto grid_barrier = [&]() -> bool {
     cta_signal(&ctl->bar);
@@ -526,45 +659,49 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
     constexpr bool APPLY_J = decltype(apply_tag)::value;
     constexpr bool DELTA = decltype(delta_tag)::value;
     ++epi;
-    const int n_tiles = nx * (y2 / TYL);
+    long long* fix = a.fix + (size_t)(epi & 1ULL) * Bs;            // this episode's fixed-point pad potentials
     if (is_z) {
-      const int grp = tid / ZT, t = tid % ZT;
-      unsigned char* gsm = phase + (size_t)grp * ZGroupSmem<NZ, EZ, TYL>::bytes;
-      double* acc = s_acc + (size_t)grp * B;
-      for (int b = t; b < B; b += ZT) acc[b] = 0.0;
-      group_sync(1 + grp, ZT);
-      for (int tile = cta + a.n_z_cta * grp; tile < n_tiles; tile += a.n_z_cta * ZG)
-        z_pass_a<NZ, EZ, TYL, LT, APPLY_J, DELTA>(a, tile, gsm, s_kz, s_twz, s_twx, s_twy, s_px, s_py, s_pl, acc, t, 1 + grp);
+      unsigned char* gsm = phase + (size_t)zgrp * ZS::bytes;
+      double* acc = RES ? reinterpret_cast<double*>(gsm + ZS::buf) : reinterpret_cast<double*>(smraw + so.acc) + (size_t)zgrp * B;
+      if (!RES) {
+        for (int b = zt; b < B; b += ZT) acc[b] = 0.0;
+        group_sync(1 + zgrp, ZT);
+      }
+      bool any = false;
+      for (int tile = my_tile; tile < n_tiles; tile += a.n_z_cta * ZG) {
+        z_pass_a<NZ, EZ, TYL, LT, RES, APPLY_J, DELTA>(a, tile, gsm, rsm, gg, s_kz, s_twz, s_twx, s_twy, s_px, s_py, s_pl, acc, zt, 1 + zgrp);
+        any = true;
+      }
+      if (RES && !any)
+        for (int b = zt; b < B; b += ZT) acc[b] = 0.0;
       __syncthreads();
+      PSTAMP();   // z1: pass A done
       for (int b = tid; b < B; b += kPersistThreads) {
         double s = 0.0;
 #pragma unroll
-        for (int q = 0; q < ZG; ++q) s += s_acc[(size_t)q * B + b];
-        a.part[(size_t)b * a.part_stride + cta] = s;
+        for (int q = 0; q < ZG; ++q)
+          s += RES ? reinterpret_cast<const double*>(phase + (size_t)q * ZS::bytes + ZS::buf)[b] : reinterpret_cast<const double*>(smraw + so.acc)[(size_t)q * B + b];
+        atomicAdd(reinterpret_cast<unsigned long long*>(fix + b), (unsigned long long)__double2ll_rn(s * kFixScale));
       }
       cta_signal(&ctl->cnt_part);
+      PSTAMP();   // z2: contributions published
       if (!cta_wait(&ctl->cnt_q, epi * (unsigned long long)a.n_b_cta, &ctl->abort, &s_ok)) return false;
-      for (int b = tid; b < B; b += kPersistThreads) s_q[b] = __ldcg(g.q + b);
-      __syncthreads();
-      for (int tile = cta + a.n_z_cta * grp; tile < n_tiles; tile += a.n_z_cta * ZG)
-        z_pass_b<NZ, EZ, TYL, LT, DELTA>(a, tile, gsm, s_kz, s_twz, s_twx, s_twy, s_px, s_py, s_q, oV, oE, t, 1 + grp);
+      PSTAMP();   // z3: charges arrived
+      for (int tile = my_tile; tile < n_tiles; tile += a.n_z_cta * ZG)
+        z_pass_b<NZ, EZ, TYL, LT, RES, DELTA>(a, tile, gsm, gg, s_kz, s_twz, s_twx, s_twy, s_px, s_py, oV, oE, zt, 1 + zgrp);
+      PSTAMP();   // z4: pass B done
     } else {
       // ---- boundary adjust on the B CTAs: rows [r0, r1) --------------------------------------------
       const int warp = tid >> 5, lane = tid & 31;
       constexpr int kWarps = kPersistThreads / 32;
+      long long* fix_next = a.fix + (size_t)((epi + 1) & 1ULL) * Bs;
       if (!cta_wait(&ctl->cnt_part, epi * (unsigned long long)a.n_z_cta, &ctl->abort, &s_ok)) return false;
-      for (int b = r0 + warp; b < r1; b += kWarps) {          // rhs_b = flag V_pad - sum_c part[b][c], fixed order
-        const double* __restrict__ row = a.part + (size_t)b * a.part_stride;
-        double s = 0.0;
-        for (int c = lane; c < a.n_z_cta; c += 32) s += __ldcg(row + c);
-#pragma unroll
-        for (int d = 16; d > 0; d >>= 1) s += __shfl_xor_sync(0xffffffffu, s, d);
-        if (lane == 0) g.rhs[b] = flag * s_vpad[b] - s;
-      }
-      cta_signal(&ctl->cnt_rhs);
-      if (!cta_wait(&ctl->cnt_rhs, epi * (unsigned long long)a.n_b_cta, &ctl->abort, &s_ok)) return false;
-      for (int b = tid; b < B; b += kPersistThreads) s_rhs[b] = __ldcg(g.rhs + b);
+      PSTAMP();   // b1: all contributions in
+      for (int b = tid; b < B; b += kPersistThreads)          // rhs = flag V_pad - V_rho|_B, every B CTA the whole vector
+        s_rhs[b] = flag * s_vpad[b] - (double)__ldcg(fix + b) * kFixInv;
+      for (int b = r0 + tid; b < r1; b += kPersistThreads) fix_next[b] = 0;   // (read last in the previous episode)
       __syncthreads();
+      PSTAMP();   // b2: rhs
       for (int row = r0 + warp; row < r1; row += kWarps) {     // Q' = Ainv rhs, one warp per row, fixed order
         double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
         int jj = lane;
@@ -589,6 +726,8 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
         if (lane == 0) g.q[row] = s;
       }
       cta_signal(&ctl->cnt_q);
+      PSTAMP();   // b3: charges published
+      PSTAMP();   // (b4: keeps the stamp count equal to the z-line CTAs')
     }
     return true;
   };
@@ -611,6 +750,17 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
       __syncthreads();
     }
   };
+  // RES: the state goes back to global memory for the next launch
+  auto save_state = [&]() {
+    if (RES && is_z && my_tile < n_tiles) {
+      const int tiles = y2 / TYL;
+      const int kx = my_tile / tiles, ky0 = (my_tile % tiles) * TYL;
+      for (int i = zt; i < NZ * TYL; i += ZT) {
+        const int kz = i / TYL, ln = i - kz * TYL;
+        g.rhat[((size_t)kx * NZ + kz) * y2 + ky0 + ln] = rsm[i];
+      }
+    }
+  };
 
   using TT = std::true_type;
   using FF = std::false_type;
@@ -623,13 +773,21 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
     plane_phase(TT{}, g.v0, g.v1, slot);
   } else {
     for (int s = 0; s < a.n_sub; ++s) {
+#ifdef WTIDE_DEBUG
+      if (tid == 0) g_fine_on = (s == 1);
+      __syncthreads();
+#endif
+      PSTAMP();   // p0: substep starts
       plane_phase(FF{}, g.v0, g.v1, 0);
+      PSTAMP();   // p1: plane units done
       if (!grid_barrier()) return;
+      PSTAMP();   // p2: barrier passed
       if (!z_phase(TT{}, FF{}, 1.0, g.v0, g.v1)) return;
       if (!grid_barrier()) return;
     }
     // H[n] from the increment of the charge since the previous output step, pads at 0 V
     if (!z_phase(FF{}, TT{}, 0.0, g.e0, g.e1)) return;
+    save_state();
     if (!grid_barrier()) return;
     plane_phase(TT{}, g.e0, g.e1, slot);
   }

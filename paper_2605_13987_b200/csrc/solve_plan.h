@@ -26,7 +26,6 @@ struct PadGroups {
 };
 PadGroups make_groups(const wt_geometry* g);
 
-constexpr int kPartStride = 160;       // >= number of z-line CTAs of the persistent kernel (SM count)
 
 // Offsets of one geometry's region inside the workspace: static tables [0, static_bytes), then state.
 struct Layout {
@@ -34,6 +33,9 @@ struct Layout {
   size_t kxd, kyd, kzd, kxf, kyf, kzf, twx, twy, twz, twxd, twyd, twzd;
   size_t static_bytes;
   size_t rhat, rhat_prev, v0, v1, m0, m1, m2, e0, e1, pl, pl_e, rhs, q, qh, part, ctl, stage;
+#ifdef WTIDE_DEBUG
+  size_t dbg;          // 256 KB of clock stamps (timing experiments)
+#endif
   size_t total;
 };
 Layout make_layout(const wt_geometry* g);
