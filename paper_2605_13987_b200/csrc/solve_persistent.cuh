@@ -106,14 +106,26 @@ __device__ __forceinline__ double2 dmulc(double2 a, double2 w) {      // a * con
 }
 
 // ------------------------------------------------------------------------------------------------
-// plane_unit: one field component on one xy-plane (k_plane_fast of solve_fast.cuh without the boundary
-// source, which the z-line phase has already added), for a GROUP of N*N/(2E) threads of the CTA.
+// plane_unit<N, E, EMIT, NC>: the xy-plane transforms of k_plane_fast (solve_fast.cuh) for a GROUP of N*N/(2E)
+// threads of the CTA, without the boundary source (the z-line phase has already added it).
+//   NC = 2  components x and y of plane z together: V~ is read once, the two transforms run interleaved (one barrier per
+//           exchange for both), and D~ = i kx J~x + i ky J~y leaves as ONE array (m0)
+//   NC = 1  component z: E~z -> J~z (m2)
+// Buffers: P[c], Q[c] (c < NC) of PlaneCfg<N>::BUF float2 each, at P0 + (2 c) BUF and P0 + (2 c + 1) BUF.
 // ------------------------------------------------------------------------------------------------
-template <int N, int E, bool EMIT>
-__device__ __forceinline__ void plane_unit(const GeomDev& g, int nz, int z, int comp, const float2* __restrict__ src, float2* P,
-                                           float2* Q, const float* s_sdt, const float* s_kx, int tid, int bar_id, int slot) {
+template <int N, int E>
+__device__ __forceinline__ void plane_load(float2 (&V)[E], const float2* __restrict__ src, int nz, int z, int tid) {
+  constexpr int Y2 = N / 2, T = N / E;
+  const int ln = tid % Y2, j = tid / Y2;
+#pragma unroll
+  for (int r = 0; r < E; ++r) V[r] = ldcg2(src + ((size_t)(j + T * r) * nz + z) * Y2 + ln);
+}
+
+template <int N, int E, bool EMIT, int NC>
+__device__ __forceinline__ void plane_unit(const GeomDev& g, int nz, int z, int comp1, const float2 (&V)[E], float2* P0,
+                                           const float* s_sdt, const float* s_kx, int tid, int bar_id, int slot) {
   using C = PlaneCfg<N>;
-  constexpr int Y2 = C::Y2, T = N / E, SX = C::SX, SU = C::SU, NT = N * N / (2 * E);
+  constexpr int Y2 = C::Y2, T = N / E, SX = C::SX, SU = C::SU, NT = N * N / (2 * E), BUF = C::BUF;
   const int ln = tid % Y2, j = tid / Y2;
   float2 w[E];
   load_twiddles<E>(w, g.twx, j);
@@ -124,94 +136,145 @@ __device__ __forceinline__ void plane_unit(const GeomDev& g, int nz, int z, int 
     for (int r = 0; r < E; ++r) sid[r] = __ldg(st + ((j + T * r) * N + 2 * ln) / 2);
   }
   const float kyv = __ldg(g.kyf + ln);
-  float2 X[E];
-#pragma unroll
-  for (int r = 0; r < E; ++r) X[r] = ldcg2(src + ((size_t)(j + T * r) * nz + z) * Y2 + ln);
-  if (comp < 2) {
-#pragma unroll
-    for (int r = 0; r < E; ++r) {
-      const float kap = (comp == 0) ? s_kx[j + T * r] : kyv;
-      X[r] = make_float2(kap * X[r].y, -kap * X[r].x);       // -i kappa V~
-    }
-  }
-  // ---- A: inverse transform along x
-  fft_stage1<E, true>(X, w);
-#pragma unroll
-  for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[q];
-  group_sync(bar_id, NT);
-  fft_stage2<E, T, true>(X, j, [&](int q, int jj) { return P[(q * T + jj) * Y2 + ln]; });
-#pragma unroll
-  for (int r = 0; r < E; ++r) Q[ln * SX + j + T * r] = X[r];
-  group_sync(bar_id, NT);
-  // Hermitian completion along y of the two packed real rows (Nyquist = 0)
+  float2 X[NC][E];
 #pragma unroll
   for (int r = 0; r < E; ++r) {
-    if (r < E / 2) {
-      const float4 ab = *reinterpret_cast<const float4*>(&Q[(j + T * r) * SX + 2 * ln]);
-      X[r] = make_float2(ab.x - ab.w, ab.y + ab.z);
+    const float2 v = V[r];
+    if constexpr (NC == 2) {
+      const float kx = s_kx[j + T * r];
+      X[0][r] = make_float2(kx * v.y, -kx * v.x);        // -i kx V~
+      X[1][r] = make_float2(kyv * v.y, -kyv * v.x);      // -i ky V~
     } else {
-      const int km = N - (j + T * r);
-      if (km == Y2) {
-        X[r] = make_float2(0.f, 0.f);
+      if (comp1 == 2) {
+        X[0][r] = v;                                     // E~z
       } else {
-        const float4 ab = *reinterpret_cast<const float4*>(&Q[km * SX + 2 * ln]);
-        X[r] = make_float2(ab.x + ab.w, ab.z - ab.y);
+        const float kap = (comp1 == 0) ? s_kx[j + T * r] : kyv;
+        X[0][r] = make_float2(kap * v.y, -kap * v.x);    // -i kappa V~
       }
     }
   }
-  // ---- B: inverse transform along y -> E at the nodes
-  fft_stage1<E, true>(X, w);
+  // ---- A: inverse transform along x
 #pragma unroll
-  for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[q];
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + (2 * c) * BUF;
+    fft_stage1<E, true>(X[c], w);
+#pragma unroll
+    for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[c][q];
+  }
   group_sync(bar_id, NT);
-  fft_stage2<E, T, true>(X, j, [&](int q, int jj) { return P[(q * T + jj) * Y2 + ln]; });
-  if constexpr (EMIT) {
-    float2* st = reinterpret_cast<float2*>(g.stage + (((size_t)slot * 3 + comp) * nz + z) * (size_t)(N * N));
 #pragma unroll
-    for (int r = 0; r < E; ++r) st[((j + T * r) * N + 2 * ln) / 2] = make_float2(X[r].x * g.inv_dt, X[r].y * g.inv_dt);
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + (2 * c) * BUF;
+    float2* Q = P + BUF;
+    fft_stage2<E, T, true>(X[c], j, [&](int q, int jj) { return P[(q * T + jj) * Y2 + ln]; });
+#pragma unroll
+    for (int r = 0; r < E; ++r) Q[ln * SX + j + T * r] = X[c][r];
+  }
+  group_sync(bar_id, NT);
+  // Hermitian completion along y of the two packed real rows (Nyquist = 0); B: inverse transform along y
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + (2 * c) * BUF;
+    float2* Q = P + BUF;
+#pragma unroll
+    for (int r = 0; r < E; ++r) {
+      if (r < E / 2) {
+        const float4 ab = *reinterpret_cast<const float4*>(&Q[(j + T * r) * SX + 2 * ln]);
+        X[c][r] = make_float2(ab.x - ab.w, ab.y + ab.z);
+      } else {
+        const int km = N - (j + T * r);
+        if (km == Y2) {
+          X[c][r] = make_float2(0.f, 0.f);
+        } else {
+          const float4 ab = *reinterpret_cast<const float4*>(&Q[km * SX + 2 * ln]);
+          X[c][r] = make_float2(ab.x + ab.w, ab.z - ab.y);
+        }
+      }
+    }
+    fft_stage1<E, true>(X[c], w);
+#pragma unroll
+    for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[c][q];
+  }
+  group_sync(bar_id, NT);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + (2 * c) * BUF;
+    fft_stage2<E, T, true>(X[c], j, [&](int q, int jj) { return P[(q * T + jj) * Y2 + ln]; });
+  }
+  if constexpr (EMIT) {
+    // (a8) H[n] = E/dt into the staging slot [slot][comp][z][y][x]
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+      const int comp = (NC == 2) ? c : comp1;
+      float2* st = reinterpret_cast<float2*>(g.stage + (((size_t)slot * 3 + comp) * nz + z) * (size_t)(N * N));
+#pragma unroll
+      for (int r = 0; r < E; ++r) st[((j + T * r) * N + 2 * ln) / 2] = make_float2(X[c][r].x * g.inv_dt, X[c][r].y * g.inv_dt);
+    }
     group_sync(bar_id, NT);                     // P is rewritten by the group's next unit
     return;
   }
+  // ---- J = (s dt_int) E nodewise (a6); C: forward transform along y
 #pragma unroll
-  for (int r = 0; r < E; ++r) {
-    X[r].x *= s_sdt[sid[r] & 0xff];
-    X[r].y *= s_sdt[sid[r] >> 8];
+  for (int c = 0; c < NC; ++c) {
+    float2* Q = P0 + (2 * c + 1) * BUF;
+#pragma unroll
+    for (int r = 0; r < E; ++r) {
+      X[c][r].x *= s_sdt[sid[r] & 0xff];
+      X[c][r].y *= s_sdt[sid[r] >> 8];
+    }
+    fft_stage1<E, false>(X[c], w);
+#pragma unroll
+    for (int q = 0; q < E; ++q) Q[(q * T + j) * Y2 + ln] = X[c][q];
   }
-  // ---- C: forward transform along y
-  fft_stage1<E, false>(X, w);
-#pragma unroll
-  for (int q = 0; q < E; ++q) Q[(q * T + j) * Y2 + ln] = X[q];
   group_sync(bar_id, NT);
-  fft_stage2<E, T, false>(X, j, [&](int q, int jj) { return Q[(q * T + jj) * Y2 + ln]; });
 #pragma unroll
-  for (int r = 0; r < E; ++r) P[(j + T * r) * SU + ln] = X[r];
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + (2 * c) * BUF;
+    float2* Q = P + BUF;
+    fft_stage2<E, T, false>(X[c], j, [&](int q, int jj) { return Q[(q * T + jj) * Y2 + ln]; });
+#pragma unroll
+    for (int r = 0; r < E; ++r) P[(j + T * r) * SU + ln] = X[c][r];
+  }
   group_sync(bar_id, NT);
-  {
+  // unpack the two real rows' half spectra; D: forward transform along x
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + (2 * c) * BUF;
+    float2* Q = P + BUF;
     const int km = (N - ln) % N;
     const bool odd = j & 1;
 #pragma unroll
     for (int r = 0; r < E; ++r) {
       const int p2 = (j + T * r) >> 1;
       const float2 zk = P[ln * SU + p2], zm = P[km * SU + p2];
-      X[r] = odd ? make_float2(0.5f * (zk.y + zm.y), 0.5f * (zm.x - zk.x))
-                 : make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
+      X[c][r] = odd ? make_float2(0.5f * (zk.y + zm.y), 0.5f * (zm.x - zk.x))
+                    : make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
     }
-  }
-  // ---- D: forward transform along x
-  fft_stage1<E, false>(X, w);
+    fft_stage1<E, false>(X[c], w);
 #pragma unroll
-  for (int q = 0; q < E; ++q) Q[(q * T + j) * Y2 + ln] = X[q];
+    for (int q = 0; q < E; ++q) Q[(q * T + j) * Y2 + ln] = X[c][q];
+  }
   group_sync(bar_id, NT);
-  fft_stage2<E, T, false>(X, j, [&](int q, int jj) { return Q[(q * T + jj) * Y2 + ln]; });
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* Q = P0 + (2 * c + 1) * BUF;
+    fft_stage2<E, T, false>(X[c], j, [&](int q, int jj) { return Q[(q * T + jj) * Y2 + ln]; });
+  }
   {
-    float2* __restrict__ dst = (comp == 0) ? g.m0 : (comp == 1) ? g.m1 : g.m2;
+    float2* __restrict__ dst = (NC == 2 || comp1 == 0) ? g.m0 : (comp1 == 1 ? g.m1 : g.m2);
 #pragma unroll
     for (int r = 0; r < E; ++r) {
       const int kx = j + T * r;
-      float2 o = X[r];
-      if (comp < 2) {
-        const float kap = (comp == 0) ? s_kx[kx] : kyv;
-        o = make_float2(-kap * o.y, kap * o.x);
+      float2 o;
+      if constexpr (NC == 2) {
+        const float kap = s_kx[kx];
+        o = make_float2(-kap * X[0][r].y - kyv * X[1][r].y, kap * X[0][r].x + kyv * X[1][r].x);    // i kx J~x + i ky J~y
+      } else {
+        o = X[0][r];
+        if (comp1 < 2) {
+          const float kap = (comp1 == 0) ? s_kx[kx] : kyv;
+          o = make_float2(-kap * o.y, kap * o.x);
+        }
       }
       dst[((size_t)kx * nz + z) * Y2 + ln] = o;
     }
@@ -243,9 +306,9 @@ constexpr double kFixInv = 1.0 / 4398046511104.0;        // (integer adds commut
 //   RES   the group owns this one tile for the whole launch: its state lives in shared memory (rsm), the inverse
 //         Green factors gg in registers, and V^_rho stays in kzb for z_pass_b
 // ------------------------------------------------------------------------------------------------
-template <int NZ, int E, int TYL, int LT, bool RES, bool APPLY_J, bool DELTA>
+template <int NZ, int E, int TYL, int LT, bool RES, bool MERGED, bool APPLY_J, bool DELTA>
 __device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigned char* gsm, double2* rsm, const double (&gg)[E / 2],
-                                         const double* s_kz, const double2* s_twz, const double2* s_twx, const double2* s_twy,
+                                         const double* s_kz, const float* s_kzf, const double2* s_twz, const double2* s_twx, const double2* s_twy,
                                          const int* s_px, const int* s_py, const int* s_pl, double* acc_pad, int tid, int bar_id) {
   using C = PencilCfg<NZ, E, TYL>;
   using S = ZGroupSmem<NZ, E, TYL>;
@@ -269,19 +332,15 @@ __device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigne
     float2 w[E];
     load_twiddles<E>(w, g.twz, j);
     float2 X[E];
-    if (f == 0) {
-      const float2* __restrict__ m0 = g.m0 + slab;
-      const float2* __restrict__ m1 = g.m1 + slab;
+    {
+      const float2* __restrict__ mf = (f == 0 ? g.m0 : g.m2) + slab;      // D~ = i kx J~x + i ky J~y | J~z
 #pragma unroll
-      for (int r = 0; r < E; ++r) {
-        const size_t o = (size_t)(j + T * r) * y2;
-        const float2 p = ldcg2(m0 + o), q = ldcg2(m1 + o);
-        X[r] = make_float2(p.x + q.x, p.y + q.y);      // D~ = i kx J~x + i ky J~y
+      for (int r = 0; r < E; ++r) X[r] = ldcg2(mf + (size_t)(j + T * r) * y2);
+      if (!MERGED && f == 0) {                                            // (plane phase with one component per unit: m0 + m1)
+        const float2* __restrict__ m1 = g.m1 + slab;
+#pragma unroll
+        for (int r = 0; r < E; ++r) { const float2 q = ldcg2(m1 + (size_t)(j + T * r) * y2); X[r].x += q.x; X[r].y += q.y; }
       }
-    } else {
-      const float2* __restrict__ m2 = g.m2 + slab;
-#pragma unroll
-      for (int r = 0; r < E; ++r) X[r] = ldcg2(m2 + (size_t)(j + T * r) * y2);
     }
     FSTAMP(1);
     fft_stage1<E, false>(X, w);
@@ -313,7 +372,7 @@ __device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigne
       double2 rr = RES ? rsm[kz * TYL + line] : rh[o];
       if constexpr (APPLY_J) {
         const float2 D = kzb[kz * TYL + line], J = kzb[(NZ + kz) * TYL + line];
-        const float kzf = (float)kzd;
+        const float kzf = s_kzf[kz];
         rr.x -= (double)(D.x - kzf * J.y);
         rr.y -= (double)(D.y + kzf * J.x);
         if (!ret) rr = make_double2(0.0, 0.0);
@@ -334,14 +393,21 @@ __device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigne
       }
       const double2 v = make_double2(src.x * ggi, src.y * ggi);
       if constexpr (RES) {                     // V^_rho and -i kz V^_rho wait in kzb for the boundary charges
-        kzb[kz * TYL + line] = make_float2((float)v.x, (float)v.y);
-        kzb[(NZ + kz) * TYL + line] = make_float2((float)(kzd * v.y), (float)(-kzd * v.x));
+        const float2 vf = make_float2((float)v.x, (float)v.y);
+        const float kzf = s_kzf[kz];
+        kzb[kz * TYL + line] = vf;
+        kzb[(NZ + kz) * TYL + line] = make_float2(kzf * vf.y, -kzf * vf.x);
       }
 #pragma unroll
       for (int l = 0; l < LT; ++l) {
         if (l < L) {
-          const double2 p = dmulc(v, s_twz[(kz * g.layers[l]) & (NZ - 1)]);      // v e^{+i kz z_l}
-          acc[l].x += p.x; acc[l].y += p.y;
+          if (g.layers[l] == 0) {                                                 // e^{+i kz 0} = 1
+            acc[l].x += v.x; acc[l].y += v.y;
+          } else {
+            const double2 w = s_twz[(kz * g.layers[l]) & (NZ - 1)];               // acc += v e^{+i kz z_l} = v conj(w)
+            acc[l].x = fma(v.x, w.x, fma(v.y, w.y, acc[l].x));
+            acc[l].y = fma(v.y, w.x, fma(-v.x, w.y, acc[l].y));
+          }
         }
       }
     }
@@ -392,7 +458,7 @@ __device__ __forceinline__ void z_pass_a(const PersistArgs& a, int tile, unsigne
 // ------------------------------------------------------------------------------------------------
 template <int NZ, int E, int TYL, int LT, bool RES, bool DELTA>
 __device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigned char* gsm, const double (&gg)[E / 2], const double* s_kz,
-                                         const double2* s_twz, const double2* s_twx, const double2* s_twy, const int* s_px, const int* s_py,
+                                         const float* s_kzf, const float2* s_twzf, const float2* s_twxf, const float2* s_twyf, const double2* s_twz, const double2* s_twx, const double2* s_twy, const int* s_px, const int* s_py,
                                          float2* __restrict__ oV, float2* __restrict__ oE, int tid, int bar_id) {
   using C = PencilCfg<NZ, E, TYL>;
   using S = ZGroupSmem<NZ, E, TYL>;
@@ -411,6 +477,40 @@ __device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigne
   double2* pls = reinterpret_cast<double2*>(gsm + S::pls);       // reused: S_l(kx, ky0 + line)
   const size_t slab = (size_t)kx * NZ * y2 + ky;
   FSTAMP(8);
+  if constexpr (RES) {
+    // the spectrum of the charges is added in fp32 below: sums of <= a few hundred terms in fp32
+    float2* csf = reinterpret_cast<float2*>(gsm + S::buf);       // [B] Q'_b e^{-i kx x_b}
+    float2* plf = reinterpret_cast<float2*>(pls);                // [L][TYL] S_l(kx, ky0 + line)
+    for (int b = tid; b < B; b += NT) {
+      const float q = (float)__ldcg(g.q + b);
+      const float2 wx = s_twxf[(kx * s_px[b]) & (nx - 1)];
+      csf[b] = make_float2(q * wx.x, q * wx.y);
+    }
+    group_sync(bar_id, NT);
+    for (int i0 = 0; i0 < L * TYL; i0 += NT / 16) {
+      const int i = i0 + tid / 16, sub = tid & 15;
+      float2 s0 = make_float2(0.f, 0.f), s1 = make_float2(0.f, 0.f);
+      if (i < L * TYL) {
+        const int l = i / TYL, kyy = ky0 + i - l * TYL;
+        int b = a.lpoff[l] + sub;
+        const int be = a.lpoff[l + 1];
+        for (; b + 16 < be; b += 32) {
+          const float2 c0 = csf[b], w0 = s_twyf[(kyy * s_py[b]) & (ny - 1)];
+          const float2 c1 = csf[b + 16], w1 = s_twyf[(kyy * s_py[b + 16]) & (ny - 1)];
+          s0.x += c0.x * w0.x - c0.y * w0.y; s0.y += c0.x * w0.y + c0.y * w0.x;
+          s1.x += c1.x * w1.x - c1.y * w1.y; s1.y += c1.x * w1.y + c1.y * w1.x;
+        }
+        if (b < be) {
+          const float2 c0 = csf[b], w0 = s_twyf[(kyy * s_py[b]) & (ny - 1)];
+          s0.x += c0.x * w0.x - c0.y * w0.y; s0.y += c0.x * w0.y + c0.y * w0.x;
+        }
+      }
+      float2 sv = make_float2(s0.x + s1.x, s0.y + s1.y);
+#pragma unroll
+      for (int d = 8; d > 0; d >>= 1) { sv.x += __shfl_xor_sync(0xffffffffu, sv.x, d); sv.y += __shfl_xor_sync(0xffffffffu, sv.y, d); }
+      if (i < L * TYL && sub == 0) plf[i] = sv;
+    }
+  } else {
   for (int b = tid; b < B; b += NT) {
     const double q = __ldcg(g.q + b);
     const double2 wx = s_twx[(kx * s_px[b]) & (nx - 1)];
@@ -432,13 +532,15 @@ __device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigne
     for (int d = 8; d > 0; d >>= 1) { s.x += __shfl_xor_sync(0xffffffffu, s.x, d); s.y += __shfl_xor_sync(0xffffffffu, s.y, d); }
     if (i < L * TYL && sub == 0) pls[i] = s;
   }
+  }
   group_sync(bar_id, NT);
   FSTAMP(9);
   if constexpr (RES) {
     // the source in fp32: kzb += (sum_l S_l e^{-i kz z_l}) gg, and the same times -i kz
+    const float2* plf = reinterpret_cast<const float2*>(pls);
     float2 sl[LT];
 #pragma unroll
-    for (int l = 0; l < LT; ++l) sl[l] = (l < L) ? make_float2((float)pls[l * TYL + line].x, (float)pls[l * TYL + line].y) : make_float2(0.f, 0.f);
+    for (int l = 0; l < LT; ++l) sl[l] = (l < L) ? plf[l * TYL + line] : make_float2(0.f, 0.f);
 #pragma unroll
     for (int i = 0; i < E / 2; ++i) {
       const int kz = j + T * (2 * i + f);
@@ -446,12 +548,11 @@ __device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigne
 #pragma unroll
       for (int l = 0; l < LT; ++l) {
         if (l < L) {
-          const double2 wd = s_twz[(kz * g.layers[l]) & (NZ - 1)];
-          const float2 wz = make_float2((float)wd.x, (float)wd.y);
+          const float2 wz = s_twzf[(kz * g.layers[l]) & (NZ - 1)];
           src.x += sl[l].x * wz.x - sl[l].y * wz.y; src.y += sl[l].x * wz.y + sl[l].y * wz.x;
         }
       }
-      const float gf = (float)gg[i], kzf = (float)s_kz[kz];
+      const float gf = (float)gg[i], kzf = s_kzf[kz];
       const float2 v = make_float2(src.x * gf, src.y * gf);
       float2 c0 = kzb[kz * TYL + line], c1 = kzb[(NZ + kz) * TYL + line];
       c0.x += v.x; c0.y += v.y;
@@ -525,7 +626,8 @@ template <int N, int EP, int NZ, int EZ, int TYL> struct PersistCfg {
   static constexpr int ZT = 2 * PencilCfg<NZ, EZ, TYL>::THREADS;    // threads of a z-line group
   static constexpr int PG = kPersistThreads / PT, ZG = kPersistThreads / ZT;
   static_assert(PG >= 1 && ZG >= 1 && PG <= 8 && ZG <= 8, "group sizes");
-  static constexpr size_t p_bytes = (size_t)PG * 2 * PlaneCfg<N>::BUF * sizeof(float2);
+  static constexpr bool MERGED = (N <= 64);                        // plane units carry the x and y components together
+  static constexpr size_t p_bytes = (size_t)PG * (MERGED ? 4 : 2) * PlaneCfg<N>::BUF * sizeof(float2);
   static constexpr size_t z_bytes = (size_t)ZG * ZGroupSmem<NZ, EZ, TYL>::bytes;
   static constexpr size_t t_bytes = (size_t)kStageSlots * 3 * N * sizeof(float);
   static constexpr size_t phase_bytes = (p_bytes > z_bytes ? p_bytes : z_bytes) > t_bytes ? (p_bytes > z_bytes ? p_bytes : z_bytes) : t_bytes;
@@ -533,14 +635,15 @@ template <int N, int EP, int NZ, int EZ, int TYL> struct PersistCfg {
 };
 
 struct PersistSmem {        // byte offsets of the table section (host and device agree through this function)
-  size_t kz, twz, twx, twy, px, py, pl, acc, sdt, kxf, phase;
+  size_t kz, kzf, twz, twzf, twx, twy, twxf, twyf, px, py, pl, acc, sdt, kxf, phase;
 };
 // acc_groups: z-line groups that need their own pad accumulators in the table section (0 in RES mode)
 __host__ __device__ inline PersistSmem persist_smem(int nx, int ny, int nz, int B, int acc_groups) {
   PersistSmem s;
   size_t p = 0;
   auto take = [&](size_t b) { size_t at = p; p = (p + b + 15) / 16 * 16; return at; };
-  s.kz = take((size_t)nz * 8); s.twz = take((size_t)nz * 16); s.twx = take((size_t)nx * 16); s.twy = take((size_t)ny * 16);
+  s.kz = take((size_t)nz * 8); s.kzf = take((size_t)nz * 4); s.twz = take((size_t)nz * 16); s.twzf = take((size_t)nz * 8);
+  s.twx = take((size_t)nx * 16); s.twy = take((size_t)ny * 16); s.twxf = take((size_t)nx * 8); s.twyf = take((size_t)ny * 8);
   s.px = take((size_t)B * 4); s.py = take((size_t)B * 4); s.pl = take((size_t)B * 4);
   s.acc = take((size_t)acc_groups * B * 8);
   s.sdt = take(256 * 4); s.kxf = take((size_t)nx * 4);
@@ -564,6 +667,10 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
   const PersistSmem so = persist_smem(nx, ny, nz, B, RES ? 0 : ZG);
   double* s_kz = reinterpret_cast<double*>(smraw + so.kz);
   double2* s_twz = reinterpret_cast<double2*>(smraw + so.twz);
+  float* s_kzf = reinterpret_cast<float*>(smraw + so.kzf);
+  float2* s_twzf = reinterpret_cast<float2*>(smraw + so.twzf);
+  float2* s_twxf = reinterpret_cast<float2*>(smraw + so.twxf);
+  float2* s_twyf = reinterpret_cast<float2*>(smraw + so.twyf);
   double2* s_twx = reinterpret_cast<double2*>(smraw + so.twx);
   double2* s_twy = reinterpret_cast<double2*>(smraw + so.twy);
   int* s_px = reinterpret_cast<int*>(smraw + so.px);
@@ -585,9 +692,9 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
   const int r0 = is_z ? 0 : min(B, brank * rows_per), r1 = is_z ? 0 : min(B, r0 + rows_per);
   const int n_tiles = nx * (y2 / TYL);
 
-  for (int i = tid; i < nz; i += kPersistThreads) { s_kz[i] = g.kzd[i]; s_twz[i] = g.twzd[i]; }
-  for (int i = tid; i < nx; i += kPersistThreads) { s_twx[i] = g.twxd[i]; s_kxf[i] = g.kxf[i]; }
-  for (int i = tid; i < ny; i += kPersistThreads) s_twy[i] = g.twyd[i];
+  for (int i = tid; i < nz; i += kPersistThreads) { s_kz[i] = g.kzd[i]; s_twz[i] = g.twzd[i]; s_kzf[i] = g.kzf[i]; s_twzf[i] = g.twz[i]; }
+  for (int i = tid; i < nx; i += kPersistThreads) { s_twx[i] = g.twxd[i]; s_kxf[i] = g.kxf[i]; s_twxf[i] = g.twx[i]; }
+  for (int i = tid; i < ny; i += kPersistThreads) { s_twy[i] = g.twyd[i]; s_twyf[i] = g.twy[i]; }
   for (int i = tid; i < 256; i += kPersistThreads) s_sdt[i] = g.sdt[i];
   for (int i = tid; i < B; i += kPersistThreads) { s_px[i] = a.pad_x[i]; s_py[i] = g.pad_y[i]; s_pl[i] = a.pad_l[i]; }
   if (!is_z) {
@@ -645,13 +752,30 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
   // ---- phases ---------------------------------------------------------------------------------
   auto plane_phase = [&](auto emit_tag, const float2* srcV, const float2* srcE, int slot) {
     constexpr bool EMIT = decltype(emit_tag)::value;
+    // units: nz "xy" units (components x and y of a plane together, twice the work) first, then nz "z" units
     const int grp = tid / PT, t = tid % PT;
-    float2* P = reinterpret_cast<float2*>(phase) + (size_t)grp * 2 * PlaneCfg<N>::BUF;
-    float2* Q = P + PlaneCfg<N>::BUF;
-    const int n_units = nz * 3, n_slots = n_cta * PG;
-    for (int u = cta * PG + grp; u < n_units; u += n_slots) {
-      const int z = u / 3, comp = u - 3 * z;
-      plane_unit<N, EP, EMIT>(g, nz, z, comp, comp == 2 ? srcE : srcV, P, Q, s_sdt, s_kxf, t, 1 + grp, slot);
+    const int n_slots = n_cta * PG;
+    // the source of the group's NEXT unit is loaded before the current unit is transformed
+    float2 V[EP], Vn[EP];
+    if constexpr (CF::MERGED) {
+      float2* P0 = reinterpret_cast<float2*>(phase) + (size_t)grp * 4 * PlaneCfg<N>::BUF;
+      int u = cta * PG + grp;
+      if (u < nz * 2) plane_load<N, EP>(V, u < nz ? srcV : srcE, nz, u < nz ? u : u - nz, t);
+      for (; u < nz * 2; u += n_slots) {
+        const int un = u + n_slots;
+        if (un < nz * 2) plane_load<N, EP>(Vn, un < nz ? srcV : srcE, nz, un < nz ? un : un - nz, t);
+        if (u < nz) plane_unit<N, EP, EMIT, 2>(g, nz, u, 0, V, P0, s_sdt, s_kxf, t, 1 + grp, slot);
+        else        plane_unit<N, EP, EMIT, 1>(g, nz, u - nz, 2, V, P0, s_sdt, s_kxf, t, 1 + grp, slot);
+#pragma unroll
+        for (int r = 0; r < EP; ++r) V[r] = Vn[r];
+      }
+    } else {
+      float2* P0 = reinterpret_cast<float2*>(phase) + (size_t)grp * 2 * PlaneCfg<N>::BUF;
+      for (int u = cta * PG + grp; u < nz * 3; u += n_slots) {
+        const int z = u / 3, comp = u - 3 * z;
+        plane_load<N, EP>(V, comp == 2 ? srcE : srcV, nz, z, t);
+        plane_unit<N, EP, EMIT, 1>(g, nz, z, comp, V, P0, s_sdt, s_kxf, t, 1 + grp, slot);
+      }
     }
   };
   // z-line phase incl. the boundary adjust; flag = 1: pads at their potentials, 0: homogeneous (increment)
@@ -669,7 +793,7 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
       }
       bool any = false;
       for (int tile = my_tile; tile < n_tiles; tile += a.n_z_cta * ZG) {
-        z_pass_a<NZ, EZ, TYL, LT, RES, APPLY_J, DELTA>(a, tile, gsm, rsm, gg, s_kz, s_twz, s_twx, s_twy, s_px, s_py, s_pl, acc, zt, 1 + zgrp);
+        z_pass_a<NZ, EZ, TYL, LT, RES, CF::MERGED, APPLY_J, DELTA>(a, tile, gsm, rsm, gg, s_kz, s_kzf, s_twz, s_twx, s_twy, s_px, s_py, s_pl, acc, zt, 1 + zgrp);
         any = true;
       }
       if (RES && !any)
@@ -688,7 +812,7 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
       if (!cta_wait(&ctl->cnt_q, epi * (unsigned long long)a.n_b_cta, &ctl->abort, &s_ok)) return false;
       PSTAMP();   // z3: charges arrived
       for (int tile = my_tile; tile < n_tiles; tile += a.n_z_cta * ZG)
-        z_pass_b<NZ, EZ, TYL, LT, RES, DELTA>(a, tile, gsm, gg, s_kz, s_twz, s_twx, s_twy, s_px, s_py, oV, oE, zt, 1 + zgrp);
+        z_pass_b<NZ, EZ, TYL, LT, RES, DELTA>(a, tile, gsm, gg, s_kz, s_kzf, s_twzf, s_twxf, s_twyf, s_twz, s_twx, s_twy, s_px, s_py, oV, oE, zt, 1 + zgrp);
       PSTAMP();   // z4: pass B done
     } else {
       // ---- boundary adjust on the B CTAs: rows [r0, r1) --------------------------------------------
