@@ -4,15 +4,21 @@
     python bench.py --gpus 1 --steps 3 --warmup 3          # our arm
     python bench.py --impl reference --steps 1 --warmup 0   # the oracle on the host cores
 
-A "step" is one pass of the whole hot path over one batch of synthetic input: wt_solve_H for the
-config-1 geometry (a0-a8) followed by wt_convolve_currents over all tracks (a9-a12).
+    python bench.py --config 3 --steps 1 --warmup 1         # the 32-geometry what-if sweep (extra row of BASELINE.md)
+    python bench.py --impl cufft                            # cuFFT-composed Euler substep (cross-check baseline only)
+
+A "step" is one pass of the whole hot path over one batch of synthetic input: wt_make_geometry (a0, host) and
+wt_solve_H (a1-a8) for the config-1 geometry followed by wt_convolve_currents over all tracks (a9-a12).
   metric / value : carrier-steps x output-samples per second of the Eq. 1.1 stage (inputs resident in HBM)
-  h_solve_s_per_geometry, stages : the H-solve part of the metric string
-  e2e            : the same Eq. 1.1 throughput with HOST (pinned) trajectory buffers and a host result
-  roofline       : dominant kernel of the step against the measured HBM peak
-  cpu_baseline   : the oracle, as it stands, on a bounded sample of the same workload
+  setup_s_per_geometry, h_solve_s_per_geometry, h_total_s_per_geometry, stages : the H-solve part of the metric string
+                   (host setup a0 timed inside the timed region, once per step; total = setup + solve)
+  e2e            : the same Eq. 1.1 throughput with HOST (pinned) trajectory buffers and a host result, and the wall
+                   clock of descriptor -> wt_make_geometry -> wt_solve_H -> synchronised table (h_solve_e2e_s)
+  roofline       : dominant stage of the step against the measured HBM peak
+  cpu_baseline   : the oracle, as it stands, on a bounded sample of the same workload (one core, and all cores for Eq. 1.1)
 Prints ONE JSON line (rank 0).
 """
+import hashlib
 import argparse
 import json
 import os
@@ -36,6 +42,26 @@ def measured_peaks():
         j = json.load(open(p))
         return float(j["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
     return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def kernel_source_hash():
+    """sha256 over the CUDA sources: profiles/r2_traffic.json holds ncu DRAM traffic for exactly one such hash"""
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2605_13987_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh", ".cpp", ".h")):
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def measured_traffic():
+    """DRAM bytes from the committed ncu --set full captures (profiles/r2_traffic.json: written by hand from the ncu
+    raw page of the command named there).  Values are only valid for the kernel sources they were captured with."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    if not os.path.exists(p):
+        return {}
+    j = json.load(open(p))
+    return j if j.get("kernel_source_hash") == kernel_source_hash() else {"stale": True, "source": j.get("source")}
 
 
 def workload(args):
@@ -116,6 +142,48 @@ def oracle_conv_sample(d, rows_of, csr, budget_s):
         terms += count_terms(sub, d["nt"])
         done = c1
     return terms, t_used, done
+
+
+_POOL_TABLE = {}
+
+
+def _conv_pool_init(table):
+    from oracle import wtide_oracle as wo  # noqa: F401  (imported once per worker, outside the timed region)
+    _POOL_TABLE["t"] = table
+
+
+def _conv_chunk(job):
+    """(worker process) the oracle's Eq. 1.1 on one chunk of carriers; the table rows were handed over at pool start"""
+    from oracle import wtide_oracle as wo
+    d, sub, pos, vel, charge = job
+    table = _POOL_TABLE["t"]
+    t0 = time.perf_counter()
+    wo.convolve_currents(lambda ix, iy, iz: table[(ix, iy, iz)], (d["nx"], d["ny"], d["nz"]), (d["lx"], d["ly"], d["lz"]), d["nt"], d["dt"],
+                         d["v_w"], sub, pos, vel, charge)
+    return time.perf_counter() - t0
+
+
+def oracle_conv_all_cores(d, table, csr, n_car):
+    """The same oracle function over a process pool, carriers split into one chunk per core (tracks and carriers are
+    independent units).  Returns (terms, wall seconds, processes)."""
+    import concurrent.futures as cf
+    import multiprocessing as mp
+    cores = os.cpu_count() or 1
+    off = np.asarray(csr["carrier_step_offsets"])
+    cuts = [n_car * k // cores for k in range(cores + 1)]
+    jobs = []
+    for k in range(cores):
+        c0, c1 = cuts[k], cuts[k + 1]
+        if c1 == c0:
+            continue
+        sl = slice(off[c0], off[c1])
+        jobs.append((d, off[c0:c1 + 1] - off[c0], csr["pos"][sl], csr["vel"][sl], csr["charge"][c0:c1]))
+    with cf.ProcessPoolExecutor(max_workers=cores, mp_context=mp.get_context("spawn"), initializer=_conv_pool_init, initargs=(table,)) as ex:
+        list(ex.map(_conv_chunk, [(d, np.zeros(2, np.int64), np.zeros((0, 3), np.float32), np.zeros((0, 3), np.float32), np.zeros(1, np.float32))] * (2 * cores)))   # workers up
+        t0 = time.perf_counter()
+        list(ex.map(_conv_chunk, jobs))
+        wall = time.perf_counter() - t0
+    return count_terms(off[:n_car + 1], d["nt"]), wall, len(jobs)
 
 
 def oracle_solve_sample(d, budget_s):
@@ -262,10 +330,13 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
 
+    if args.config == 3:
+        return run_sweep(args, wt, dev, world, rank)
     d = workload(args)
     nt = d["nt"]
     n_nodes = d["nx"] * d["ny"] * d["nz"]
     g = wt.wt_make_geometry(d)
+    plan = wt.wt_describe_plan(g)
     n_sub = wt.wt_query(g, wt.WT_Q_SUBSTEPS)
     n_pads = wt.wt_query(g, wt.WT_Q_N_PADS)
     side = wt._stream(dev)
@@ -292,10 +363,17 @@ def run_ours(args):
     ws_conv = torch.empty(wt.wt_conv_workspace_bytes(g, args.tracks, n_car, True) + 256, dtype=torch.uint8, device=dev)
     out = torch.empty((args.tracks, nt), dtype=torch.float32, device=dev)
 
+    setup_times = []
+
     def step(ev=None):
+        # a0: host setup of the geometry, every step (the handle of the previous step is dropped)
+        t0 = time.perf_counter()
+        gk = wt.wt_make_geometry(d)
+        setup_times.append(time.perf_counter() - t0)
+        gsk = [gk] * K
         if ev:
             ev[0].record(side)
-        wt.wt_solve_H(gs, H=H, workspace=ws_solve, device=dev)
+        wt.wt_solve_H(gsk, H=H, workspace=ws_solve, device=dev)
         if ev:
             ev[1].record(side)
         wt.wt_convolve_currents(g, H[0], csr["track_carrier_offsets"], csr["carrier_step_offsets"], csr["pos"], csr["vel"],
@@ -311,6 +389,7 @@ def run_ours(args):
     for _ in range(args.warmup):
         step()
     barrier()
+    setup_times.clear()
     launches0 = wt.wt_launch_count()
     evs = [[torch.cuda.Event(enable_timing=True) for _ in range(3)] for _ in range(args.steps)]
     with ClockSampler(local) as clk:
@@ -323,6 +402,16 @@ def run_ours(args):
     solve_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
     conv_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
     step_ms = float(np.mean([e[0].elapsed_time(e[2]) for e in evs]))
+    setup_s = float(np.mean(setup_times))
+    # end to end for the solve: descriptor -> handle -> synchronised table, wall clock
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    ge = wt.wt_make_geometry(d)
+    wt.wt_solve_H([ge], H=H[:1], workspace=ws_solve, device=dev)
+    torch.cuda.synchronize()
+    first_row = H[0][0, 0, 0].cpu()                      # (device -> host read of a result row)
+    h_solve_e2e_s = time.perf_counter() - t0
+    del first_row
 
     # ---- e2e: Eq. 1.1 through the C ABI with host buffers (pinned), copies inside the timed region.
     # The tracks go in batches (they are independent units): the host->device copy of batch b + 1
@@ -391,22 +480,31 @@ def run_ours(args):
         # DRAM bytes from the ncu --set full captures of this workload (profiles/r1_solve.md, profiles/r1_conv.md):
         # solve = 35.9 MB per substep in the cold-cache capture of its three kernels (an upper bound: in the replayed
         # graph the working set is L2-resident); Eq. 1.1 = 154.4 GB per call at 1000 tracks x 1000 carriers.
-        default_workload = (args.config == 1 and args.tracks == 1000 and args.carriers == 1000 and not args.grid and not args.nt)
-        traffic_solve = 35.9e6 * n_sub * (nt - 1) if (default_workload and K == 1) else None
-        traffic_conv = 154.4e9 if default_workload else None
-        roof = {"bound": "hbm", "kernel": "wt_solve_H (k_plane_fast + k_pencil2 + k_boundary_fast, all substeps)" if dominant_is_solve
+        default_workload = (args.tracks == 1000 and args.carriers == 1000 and not args.grid and not args.nt and K == 1)
+        tr = measured_traffic().get("configs[%d]" % args.config, {}) if default_workload else {}
+        traffic_solve = tr["solve_dram_bytes_per_substep"] * n_sub * (nt - 1) if "solve_dram_bytes_per_substep" in tr else None
+        traffic_conv = tr.get("conv_dram_bytes")
+        fma_peak = wt.wt_measure_fp32_fma(dev)
+        roof = {"bound": "hbm", "kernel": ("wt_solve_H, all substeps -- " + plan) if dominant_is_solve
                 else "k_conv_systolic", "achieved": solve_gbs if dominant_is_solve else conv_gbs, "peak": peak, "unit": "GB/s",
                 "frac": (solve_gbs if dominant_is_solve else conv_gbs) / peak,
                 "traffic": traffic_solve if dominant_is_solve else traffic_conv, "peak_source": peak_kind,
-                "algorithmic_bytes": alg_solve_bytes if dominant_is_solve else alg_conv_bytes}
+                "traffic_source": "profiles/r2_traffic.json (ncu --set full, same kernel sources)" if tr else None,
+                "algorithmic_bytes": alg_solve_bytes if dominant_is_solve else alg_conv_bytes,
+                "fp32_fma_peak_tflops_measured": fma_peak}
         stages = {"solve_ms": solve_ms, "conv_ms": conv_ms,
                   "solve": {"algorithmic_bytes": alg_solve_bytes, "achieved_gbs": solve_gbs, "frac": solve_gbs / peak,
                             "traffic": traffic_solve,
                             "n_sub": n_sub, "substeps": n_sub * (nt - 1), "us_per_substep": 1e3 * solve_ms / (n_sub * (nt - 1)) / K, "pads": n_pads,
                             "lock_step_geometries": K},
                   "conv": {"algorithmic_bytes": alg_conv_bytes, "no_reuse_gather_bytes": 96 * terms, "achieved_gbs": conv_gbs,
-                           "frac": conv_gbs / peak, "traffic": traffic_conv, "carriers": n_car, "carrier_steps": n_steps_total,
+                           "frac": conv_gbs / peak, "traffic": traffic_conv,
+                           "dram_frac": (traffic_conv / (conv_ms * 1e-3) / 1e9 / peak) if traffic_conv else None,
+                           "fp32_flops": 48 * terms, "fp32_frac_of_measured_fma_peak": 48 * terms / (conv_ms * 1e-3) / 1e12 / fma_peak,
+                           "carriers": n_car, "carrier_steps": n_steps_total,
                            "mean_steps": n_steps_total / max(1, n_car)}}
+        stages["solve"]["plan"] = plan
+        stages["setup_s"] = setup_s
         line = {"metric": METRIC, "value": total_terms / (conv_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f32", "data": "synthetic",
@@ -416,11 +514,15 @@ def run_ours(args):
                               d["nx"], d["ny"], d["nz"], nt, d["dt"], args.tracks, args.carriers),
                            "l2": "inputs larger than L2 (H table %.2f GB, trajectories %.2f GB)" % (n_nodes * nt * 12 / 1e9, n_steps_total * 24 / 1e9),
                            "parallelism": "replicas, tracks sharded" if world > 1 else "single GPU"},
-                "h_solve_s_per_geometry": solve_ms * 1e-3 / K, "step_value": total_terms / (step_ms * 1e-3), "stages": stages,
+                "setup_s_per_geometry": setup_s, "h_solve_s_per_geometry": solve_ms * 1e-3 / K,
+                "h_total_s_per_geometry": setup_s + solve_ms * 1e-3 / K,
+                "step_value": total_terms / (step_ms * 1e-3 + setup_s), "stages": stages,
                 "roofline": roof,
                 "e2e": {"value": total_terms / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                         "what": "Eq. 1.1 stage with pinned host trajectories in, host currents out, %d track batches, copies overlapped with the kernels" % n_batches,
-                        "max_dev_from_one_call_result_rel_peak": e2e_dev},
+                        "max_dev_from_one_call_result_rel_peak": e2e_dev,
+                        "h_solve_e2e_s": h_solve_e2e_s,
+                        "h_solve_e2e_what": "descriptor -> wt_make_geometry -> wt_solve_H -> synchronize -> one table row on the host, wall clock"},
                 "gpu_launches": int(launches), "clocks": clk.summary(), "wall_s_timed_region": wall}
         if not args.no_cpu_baseline and world == 1:
             # the oracle on a bounded sample of the same workload (first carriers of track 0), rows of
@@ -442,7 +544,10 @@ def run_ours(args):
             table = {t: rows[i] for i, t in enumerate(ids)}
             o_terms, o_t, o_car = oracle_conv_sample(d, lambda ix, iy, iz: table[(ix, iy, iz)], sample, args.ref_budget)
             per_sub, nsubs, _, _ = oracle_solve_sample(d, args.ref_budget)
+            a_terms, a_wall, a_procs = oracle_conv_all_cores(d, table, sample, o_car)
             line["cpu_baseline"] = {"value": o_terms / o_t, "unit": UNIT, "cores": 1, "kind": "oracle",
+                                    "all_cores": {"value": a_terms / a_wall, "unit": UNIT, "cores": a_procs,
+                                                  "what": "the same carriers of Eq. 1.1 split over one oracle process per host core"},
                                     "sample": "first %d carriers (%.1f s) for Eq. 1.1; %d Euler substeps on the full grid (%.2f s each) "
                                               "-> H solve extrapolated to %.0f s per geometry" % (o_car, o_t, nsubs, per_sub, per_sub * n_sub * (nt - 1)),
                                     "h_solve_s_per_geometry_extrapolated": per_sub * n_sub * (nt - 1), "host_cores_available": os.cpu_count()}
@@ -451,15 +556,188 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+# --------------------------------------------------------------------------------------------------
+# config 3: the 32-geometry what-if sweep (PAPER.md:15 "what-if studies on sensor geometry", :137-141 the bias
+# diameter scan).  Every cell: host setup (a0) -> wt_solve_H -> 200 tracks x 1000 carriers through Eq. 1.1.
+# The setup of cell i + 1 runs on a host thread while the GPU works on cell i.  One table (6.44 GB) is reused.
+# --------------------------------------------------------------------------------------------------
+def run_sweep(args, wt, dev, world, rank):
+    import concurrent.futures as cf
+
+    import torch
+    import torch.distributed as dist
+
+    from wtide_inputs import carriers_on_tracks, field_drift, make_tracks, reduced_desc
+    from wtide_inputs.configs import sweep_descs
+    descs = sweep_descs()
+    if args.nt:
+        descs = [reduced_desc(dd, nt=args.nt) for dd in descs]
+    cells = [int(c) for c in args.cells.split(",")] if args.cells else list(range(len(descs)))
+    cells = cells[rank::world]
+    n_tracks = 200 if args.tracks == 1000 else args.tracks
+    d0 = descs[0]
+    nt, n_nodes = d0["nt"], d0["nx"] * d0["ny"] * d0["nz"]
+    side = wt._stream(dev)
+    H = torch.empty((d0["nx"], d0["ny"], d0["nz"], nt, 3), dtype=torch.float32, device=dev)
+    out = torch.empty((n_tracks, nt), dtype=torch.float32, device=dev)
+    pool = cf.ThreadPoolExecutor(max_workers=1)
+
+    def timed_setup(dd):
+        t0 = time.perf_counter()
+        gg = wt.wt_make_geometry(dd)
+        return gg, time.perf_counter() - t0
+
+    def one_pass(record):
+        rows = []
+        fut = pool.submit(timed_setup, descs[cells[0]])
+        ws = None
+        for k, ci in enumerate(cells):
+            g, t_setup = fut.result()
+            if k + 1 < len(cells):
+                fut = pool.submit(timed_setup, descs[cells[k + 1]])        # overlaps with this cell's GPU work
+            dd = descs[ci]
+            need = wt.wt_query(g, wt.WT_Q_SOLVE_WORKSPACE_BYTES) + 256
+            if ws is None or ws.numel() < need:
+                ws = torch.empty(need, dtype=torch.uint8, device=dev)
+            e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            e[0].record(side)
+            wt.wt_solve_H([g], H=[H], workspace=ws, device=dev)
+            e[1].record(side)
+            torch.cuda.synchronize()
+            # inputs of Eq. 1.1 (outside every timed quantity): drift in the static field of this table
+            e_static = H.view(n_nodes, nt, 3).sum(dim=1).mul_(dd["dt"]).view(dd["nx"], dd["ny"], dd["nz"], 3)
+            tracks = make_tracks(3, n_tracks, dd, 10.0)
+            start, sign, charge, toff = carriers_on_tracks(tracks, args.carriers, dd)
+            csr = field_drift(e_static, dd, start, sign, charge, toff)
+            del e_static
+            n_car = csr["carrier_step_offsets"].numel() - 1
+            wsc = torch.empty(wt.wt_conv_workspace_bytes(g, n_tracks, n_car, True) + 256, dtype=torch.uint8, device=dev)
+            torch.cuda.synchronize()
+            e[2].record(side)
+            wt.wt_convolve_currents(g, H, csr["track_carrier_offsets"], csr["carrier_step_offsets"], csr["pos"], csr["vel"], csr["charge"],
+                                    per_track=True, out=out, workspace=wsc)
+            e[3].record(side)
+            torch.cuda.synchronize()
+            if record:
+                terms = count_terms(csr["carrier_step_offsets"].cpu().numpy(), nt)
+                n_sub = wt.wt_query(g, wt.WT_Q_SUBSTEPS)
+                rows.append({"cell": ci, "pitch_um": dd["lx"], "bias_radius_um": dd["columns"][1]["radius"], "resistivity_ohm_cm": dd["columns"][0]["resistivity"],
+                             "pads": wt.wt_query(g, wt.WT_Q_N_PADS), "n_sub": n_sub, "plan": wt.wt_describe_plan(g).split(":")[0],
+                             "setup_s": t_setup, "solve_s": e[0].elapsed_time(e[1]) * 1e-3, "conv_s": e[2].elapsed_time(e[3]) * 1e-3,
+                             "terms": terms, "finite": bool(torch.isfinite(out).all())})
+        return rows
+
+    for _ in range(min(args.warmup, 1)):
+        one_pass(False)
+    launches0 = wt.wt_launch_count()
+    with ClockSampler(int(dev.split(":")[1])) as clk:
+        t0 = time.perf_counter()
+        rows = one_pass(True)
+        wall = time.perf_counter() - t0
+    launches = wt.wt_launch_count() - launches0
+    peak, peak_kind = measured_peaks()
+    tot = {k: sum(r[k] for r in rows) for k in ("setup_s", "solve_s", "conv_s", "terms")}
+    groups = {}
+    for r in rows:
+        gk = groups.setdefault(str(r["n_sub"]), {"cells": 0, "solve_s": 0.0, "alg_bytes": 0.0, "setup_s": 0.0})
+        gk["cells"] += 1
+        gk["solve_s"] += r["solve_s"]
+        gk["setup_s"] += r["setup_s"]
+        gk["alg_bytes"] += (60 * n_nodes * r["n_sub"] + 40 * n_nodes) * (nt - 1) + 40 * n_nodes
+    for gk in groups.values():
+        gk["solve_frac_of_hbm_roofline"] = gk["alg_bytes"] / gk["solve_s"] / 1e9 / peak
+        gk["solve_s_per_geometry"] = gk["solve_s"] / gk["cells"]
+    vals = torch.tensor([tot["setup_s"], tot["solve_s"], tot["conv_s"]], dtype=torch.float64, device=dev)
+    work = torch.tensor([float(tot["terms"]), float(len(rows))], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(vals, op=dist.ReduceOp.MAX)
+        dist.all_reduce(work, op=dist.ReduceOp.SUM)
+    if rank == 0:
+        setup_s, solve_s, conv_s = (float(v) for v in vals.cpu())
+        terms, n_geo = (float(v) for v in work.cpu())
+        per_rank_geo = len(rows)
+        alg = sum(gk["alg_bytes"] for gk in groups.values())
+        line = {"metric": METRIC, "value": terms / conv_s, "unit": UNIT, "n_gpus": world, "steps": 1, "warmup": min(args.warmup, 1),
+                "ms_per_step": 1e3 * (setup_s + solve_s + conv_s), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f32", "data": "synthetic",
+                "config": {"workload": "configs[3] what-if sweep: %d square cells (pitch x bias radius x resistivity), grid %dx%dx%d, nt=%d, %d tracks x %d carriers per geometry"
+                           % (int(n_geo), d0["nx"], d0["ny"], d0["nz"], nt, n_tracks, args.carriers),
+                           "l2": "inputs larger than L2 (H table %.2f GB per geometry)" % (n_nodes * nt * 12 / 1e9),
+                           "parallelism": "replicas, geometries sharded" if world > 1 else "single GPU"},
+                "setup_s_per_geometry": setup_s / per_rank_geo, "h_solve_s_per_geometry": solve_s / per_rank_geo,
+                "conv_s_per_geometry": conv_s / per_rank_geo, "h_total_s_per_geometry": (setup_s + solve_s) / per_rank_geo,
+                "s_per_geometry_all_stages": (setup_s + solve_s + conv_s) / per_rank_geo,
+                "wall_s_sweep_incl_input_generation": wall,
+                "roofline": {"bound": "hbm", "kernel": "wt_solve_H over the sweep (per-cell plans in `cells`)", "achieved": alg / solve_s / 1e9,
+                             "peak": peak, "unit": "GB/s", "frac": alg / solve_s / 1e9 / peak, "traffic": None, "peak_source": peak_kind,
+                             "algorithmic_bytes": alg},
+                "by_n_sub": groups, "cells": rows, "gpu_launches": int(launches), "clocks": clk.summary(),
+                "e2e": {"value": terms / (setup_s + solve_s + conv_s), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                        "what": "terms per second of the whole sweep incl. host setup and the H solves (trajectories are generated on the device "
+                                "from each table: no host buffers in this workload)"}}
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+# --------------------------------------------------------------------------------------------------
+# --impl cufft: the Euler substep composed from cuFFT 3-D transforms (torch.fft) and elementwise kernels, as the
+# paper's own port does ("the 3D FFT implementation shipped with CUDA" + a |k|^2 kernel).  A
+# cross-check BASELINE for the fused kernels' head-room (~200 N bytes per substep), not product code:
+# no boundary solve, fp32 state.
+# --------------------------------------------------------------------------------------------------
+def run_cufft(args):
+    import torch
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    d = workload(args)
+    dev = "cuda:0"
+    nx, ny, nz = d["nx"], d["ny"], d["nz"]
+    N = nx * ny * nz
+    kx = (2 * np.pi * np.fft.fftfreq(nx, d["lx"] / nx)).astype(np.float32)
+    ky = (2 * np.pi * np.fft.fftfreq(ny, d["ly"] / ny)).astype(np.float32)
+    kz = (2 * np.pi * np.fft.rfftfreq(nz, d["lz"] / nz)).astype(np.float32)
+    KX = torch.tensor(kx, device=dev)[:, None, None]
+    KY = torch.tensor(ky, device=dev)[None, :, None]
+    KZ = torch.tensor(kz, device=dev)[None, None, :]
+    k2 = KX * KX + KY * KY + KZ * KZ
+    ginv = torch.where(k2 > 0, 1.0 / k2, torch.zeros_like(k2))
+    sig = (torch.rand((nx, ny, nz), device=dev) < 0.08).float() * 1e-2
+    rh = torch.fft.rfftn(torch.randn((nx, ny, nz), device=dev))
+
+    def substep(rh):
+        vh = rh * ginv
+        acc = torch.zeros_like(rh)
+        for K in (KX, KY, KZ):
+            e = torch.fft.irfftn(-1j * K * vh, s=(nx, ny, nz))
+            acc += 1j * K * torch.fft.rfftn(sig * e)
+        return rh - acc
+    n_rep = 50
+    for _ in range(5):
+        rh = substep(rh)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(n_rep):
+        rh = substep(rh)
+    e1.record()
+    torch.cuda.synchronize()
+    us = e0.elapsed_time(e1) * 1e3 / n_rep
+    peak, peak_kind = measured_peaks()
+    print(json.dumps({"impl": "cufft", "what": "Euler substep composed from torch.fft (cuFFT) rfftn/irfftn + elementwise kernels, no boundary solve, fp32",
+                      "grid": [nx, ny, nz], "us_per_substep": us, "frac_of_60N_hbm_roofline": 60 * N / (us * 1e-6) / 1e9 / peak,
+                      "peak": peak, "peak_source": peak_kind}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference", "cufft"])
     ap.add_argument("--tracks", type=int, default=1000, help="MIP tracks per GPU")
     ap.add_argument("--carriers", type=int, default=1000, help="macro-carriers per track")
-    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 4],
+    ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4],
                     help="BASELINE.json config whose geometry, grid and nt are used (default 1 = the bench line; 2 and 4 are "
                          "measured as extra rows of BASELINE.md with one batch of tracks, see DESIGN.md)")
     ap.add_argument("--batch", type=int, default=1, help="lock-step copies of the geometry per wt_solve_H call (extra measurement; 1 = bench line)")
@@ -467,9 +745,17 @@ def main():
     ap.add_argument("--nt", type=int, default=0, help="override nt (debug only)")
     ap.add_argument("--ref-budget", type=float, default=10.0, help="seconds of oracle work per leg")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cells", default="", help="config 3 only: comma-separated indices of the sweep cells to run (default: all 32)")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # launched without torchrun: start the N ranks ourselves (one process per GPU, replicas: DESIGN.md section 9)
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(29500 + os.getpid() % 2000), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
     if args.impl == "reference":
         run_reference(args)
+    elif args.impl == "cufft":
+        run_cufft(args)
     else:
         run_ours(args)
 

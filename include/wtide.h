@@ -150,6 +150,11 @@ int wt_get_array(const wt_geometry* geom, int what, void* host_out, size_t bytes
  * kernel chain, and which kernels), for logs and bench labels.  Needs no GPU for the chain; `out` is NUL-terminated. */
 int wt_describe_plan(const wt_geometry* geom, char* out, size_t out_bytes);
 
+/* Measured FP32 FMA rate of the current device in TFLOP/s (2 flops per FMA), for roofline reports: a short
+ * register-resident FMA kernel on every SM, best of 5.  The ONLY call that waits for the device.
+ * scratch_dev: device scratch of >= 1.25 MB. */
+int wt_measure_fp32_fma(void* scratch_dev, size_t scratch_bytes, void* cuda_stream, double* tflops);
+
 /* Number of CUDA kernels this process has launched through libwtide so far (bench.py reports the
  * difference over its timed region as "gpu_launches"). */
 int64_t wt_launch_count(void);

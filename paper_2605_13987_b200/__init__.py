@@ -21,7 +21,7 @@ WT_Q_N_NODES, WT_Q_N_CONDUCTING, WT_Q_N_PAD_LAYERS, WT_Q_NT = 5, 6, 7, 8
 WT_A_COLUMN_ID, WT_A_PAD_NODES, WT_A_PAD_POTENTIAL, WT_A_AINV, WT_A_GT, WT_A_GZT = 1, 2, 3, 4, 5, 6
 
 EXPORTS = ("wt_make_geometry", "wt_solve_H", "wt_convolve_currents", "wt_free", "wt_trajectory_nodes",
-           "wt_conv_workspace_bytes", "wt_query", "wt_get_array", "wt_last_error", "wt_launch_count", "wt_describe_plan")
+           "wt_conv_workspace_bytes", "wt_query", "wt_get_array", "wt_last_error", "wt_launch_count", "wt_describe_plan", "wt_measure_fp32_fma")
 
 
 class wt_column(C.Structure):
@@ -65,6 +65,8 @@ def _load():
     lib.wt_get_array.argtypes = [vp, C.c_int, vp, sz]
     lib.wt_describe_plan.argtypes = [vp, C.c_char_p, sz]
     lib.wt_describe_plan.restype = C.c_int
+    lib.wt_measure_fp32_fma.argtypes = [vp, sz, vp, C.POINTER(C.c_double)]
+    lib.wt_measure_fp32_fma.restype = C.c_int
     lib.wt_last_error.restype = C.c_char_p
     lib.wt_launch_count.restype = C.c_int64
     for n in ("wt_make_geometry", "wt_solve_H", "wt_convolve_currents", "wt_trajectory_nodes",
@@ -233,6 +235,16 @@ def wt_describe_plan(geom: Geometry) -> str:
     buf = C.create_string_buffer(512)
     _check(_lib.wt_describe_plan(geom.handle, buf, len(buf)))
     return buf.value.decode()
+
+
+def wt_measure_fp32_fma(device="cuda:0") -> float:
+    """Measured FP32 FMA rate of the device in TFLOP/s."""
+    import torch
+    scratch = torch.empty(4 << 20, dtype=torch.uint8, device=device)
+    out = C.c_double()
+    with torch.cuda.device(device):
+        _check(_lib.wt_measure_fp32_fma(scratch.data_ptr(), scratch.numel(), _stream(device).cuda_stream, C.byref(out)))
+    return out.value
 
 
 def wt_launch_count() -> int:

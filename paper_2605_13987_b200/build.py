@@ -21,6 +21,7 @@ UNITS = {
     "csrc/solve_persistent.cu": HEADERS,
     "csrc/conv.cu": ["csrc/geometry.h", "../include/wtide.h"],
     "csrc/static_field.cu": HEADERS,
+    "csrc/peaks.cu": ["csrc/geometry.h", "../include/wtide.h"],
 }
 SOURCES = [u for u in UNITS if os.path.exists(os.path.join(HERE, u))]
 DEPS = SOURCES + [h for h in HEADERS if os.path.exists(os.path.join(HERE, h))]
