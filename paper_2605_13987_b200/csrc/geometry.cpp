@@ -399,6 +399,7 @@ extern "C" int wt_make_geometry(const wt_geometry_desc* d, wt_geometry** out) {
       for (int j = 0; j < B; ++j) g->ainv[(size_t)i * B + j] = a[(size_t)i * B + j] - ui * u[j];
     }
   }
+  if (!wt_build_solve_cache(g)) { delete g; wt_set_error("wt_make_geometry: out of host memory"); return WT_ENOMEM; }
   *out = g;
   wt_set_error("");
   return WT_OK;

@@ -39,3 +39,4 @@ extern std::atomic<long long> g_wt_launches;   // kernels launched by this proce
 void wt_set_error(const std::string& msg);
 bool wt_valid(const wt_geometry* g);
 bool wt_is_2a3b(int n);
+bool wt_build_solve_cache(wt_geometry* g);   // solve.cu: what wt_solve_H uploads, packed once per handle (host only)

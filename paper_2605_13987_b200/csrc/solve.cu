@@ -15,8 +15,8 @@
 // Two executions of these phases exist (solve_plan.h): the persistent kernel (one cooperative launch per
 // output step, solve_persistent.cu) for the power-of-two grids of the BASELINE configs, and the kernel chain
 // (one kernel per phase, CUDA graph, solve_chain.cu) for everything else.  A batch is split between them per
-// geometry.  The static tables of a geometry are packed once per handle into one pinned host blob and reach
-// the workspace with a single asynchronous copy per call.
+// geometry.  The static tables of a geometry are packed once per handle (by wt_make_geometry) into one host blob and
+// reach the workspace with a single copy per call.
 #include <cuda_runtime.h>
 
 #include <algorithm>
@@ -109,12 +109,8 @@ namespace {
 struct SolveCache {
   PadGroups pg;
   Layout lo;
-  char* blob = nullptr;
-  bool pinned = false;
-  ~SolveCache() {
-    if (blob && pinned) cudaFreeHost(blob);
-    else std::free(blob);
-  }
+  char* blob = nullptr;        // pageable: packed by wt_make_geometry (host only), one cudaMemcpyAsync per wt_solve_H call
+  ~SolveCache() { std::free(blob); }
 };
 
 template <typename T>
@@ -129,9 +125,7 @@ SolveCache* get_cache(wt_geometry* g) {
   c->lo = make_layout(g);
   const Layout& lo = c->lo;
   const PadGroups& pg = c->pg;
-  void* p = nullptr;
-  if (cudaMallocHost(&p, lo.static_bytes) == cudaSuccess) { c->blob = (char*)p; c->pinned = true; }
-  else { cudaGetLastError(); c->blob = (char*)std::malloc(lo.static_bytes); }
+  c->blob = (char*)std::malloc(lo.static_bytes);
   if (!c->blob) return nullptr;
   std::memset(c->blob, 0, lo.static_bytes);
   char* b = c->blob;
@@ -182,6 +176,9 @@ bool use_persistent(const wt_geometry* g) {
 }  // namespace wt
 
 using namespace wt;
+
+// called at the end of wt_make_geometry (host work, part of the setup a0): pad groups, layout, packed static tables
+bool wt_build_solve_cache(wt_geometry* g) { return get_cache(g) != nullptr; }
 
 // bytes wt_solve_H needs for this geometry (its region + one descriptor slot + the step counter)
 size_t wt_solve_workspace_bytes(const wt_geometry* g) { return make_layout(g).total + 4096; }

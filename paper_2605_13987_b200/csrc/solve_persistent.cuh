@@ -281,6 +281,174 @@ __device__ __forceinline__ void plane_unit(const GeomDev& g, int nz, int z, int 
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// plane_unit3<N, E, EMIT>: ALL THREE components of plane z in one pass of a group (N <= 64): V~ and E~z are read
+// once, the three transforms run interleaved between shared barriers, D~ = i kx J~x + i ky J~y and J~z leave as two
+// arrays (m0, m2).  One exchange buffer per component (PlaneCfg<N>::BUF float2 each, at P0 + c BUF), reused in place:
+// a barrier separates the last read of an exchange from the first write of the next.
+// With nz plane units for about as many groups the plane phase is a single round.
+// ------------------------------------------------------------------------------------------------
+template <int N, int E, bool EMIT>
+__device__ __forceinline__ void plane_unit3(const GeomDev& g, int nz, int z, const float2 (&VV)[E], const float2 (&VE)[E], float2* P0,
+                                            const float* s_sdt, const float* s_kx, int tid, int bar_id, int slot) {
+  using C = PlaneCfg<N>;
+  constexpr int Y2 = C::Y2, T = N / E, SX = C::SX, SU = C::SU, NT = N * N / (2 * E), BUF = C::BUF, NC = 3;
+  const int ln = tid % Y2, j = tid / Y2;
+  float2 w[E];
+  load_twiddles<E>(w, g.twx, j);
+  unsigned short sid[E];
+  if (!EMIT) {
+    const unsigned short* st = reinterpret_cast<const unsigned short*>(g.sig_t + (size_t)z * N * N);
+#pragma unroll
+    for (int r = 0; r < E; ++r) sid[r] = __ldg(st + ((j + T * r) * N + 2 * ln) / 2);
+  }
+  const float kyv = __ldg(g.kyf + ln);
+  float2 X[NC][E];
+#pragma unroll
+  for (int r = 0; r < E; ++r) {
+    const float2 v = VV[r];
+    const float kx = s_kx[j + T * r];
+    X[0][r] = make_float2(kx * v.y, -kx * v.x);        // -i kx V~
+    X[1][r] = make_float2(kyv * v.y, -kyv * v.x);      // -i ky V~
+    X[2][r] = VE[r];                                   // E~z
+  }
+  // ---- A: inverse transform along x
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+    fft_stage1<E, true>(X[c], w);
+#pragma unroll
+    for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[c][q];
+  }
+  group_sync(bar_id, NT);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+    fft_stage2<E, T, true>(X[c], j, [&](int q, int jj) { return P[(q * T + jj) * Y2 + ln]; });
+  }
+  group_sync(bar_id, NT);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+#pragma unroll
+    for (int r = 0; r < E; ++r) P[ln * SX + j + T * r] = X[c][r];        // transposed: [ky][x]
+  }
+  group_sync(bar_id, NT);
+  // Hermitian completion along y of the two packed real rows (Nyquist = 0)
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+#pragma unroll
+    for (int r = 0; r < E; ++r) {
+      if (r < E / 2) {
+        const float4 ab = *reinterpret_cast<const float4*>(&P[(j + T * r) * SX + 2 * ln]);
+        X[c][r] = make_float2(ab.x - ab.w, ab.y + ab.z);
+      } else {
+        const int km = N - (j + T * r);
+        if (km == Y2) {
+          X[c][r] = make_float2(0.f, 0.f);
+        } else {
+          const float4 ab = *reinterpret_cast<const float4*>(&P[km * SX + 2 * ln]);
+          X[c][r] = make_float2(ab.x + ab.w, ab.z - ab.y);
+        }
+      }
+    }
+    fft_stage1<E, true>(X[c], w);           // B: inverse transform along y
+  }
+  group_sync(bar_id, NT);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+#pragma unroll
+    for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[c][q];
+  }
+  group_sync(bar_id, NT);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+    fft_stage2<E, T, true>(X[c], j, [&](int q, int jj) { return P[(q * T + jj) * Y2 + ln]; });
+  }
+  if constexpr (EMIT) {
+    // (a8) H[n] = E/dt into the staging slot [slot][comp][z][y][x]
+#pragma unroll
+    for (int c = 0; c < NC; ++c) {
+      float2* st = reinterpret_cast<float2*>(g.stage + (((size_t)slot * 3 + c) * nz + z) * (size_t)(N * N));
+#pragma unroll
+      for (int r = 0; r < E; ++r) st[((j + T * r) * N + 2 * ln) / 2] = make_float2(X[c][r].x * g.inv_dt, X[c][r].y * g.inv_dt);
+    }
+    group_sync(bar_id, NT);                     // the buffers are rewritten by the group's next unit
+    return;
+  }
+  // ---- J = (s dt_int) E nodewise (a6); C: forward transform along y
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+#pragma unroll
+    for (int r = 0; r < E; ++r) {
+      X[c][r].x *= s_sdt[sid[r] & 0xff];
+      X[c][r].y *= s_sdt[sid[r] >> 8];
+    }
+    fft_stage1<E, false>(X[c], w);
+  }
+  group_sync(bar_id, NT);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+#pragma unroll
+    for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[c][q];
+  }
+  group_sync(bar_id, NT);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+    fft_stage2<E, T, false>(X[c], j, [&](int q, int jj) { return P[(q * T + jj) * Y2 + ln]; });
+  }
+  group_sync(bar_id, NT);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+#pragma unroll
+    for (int r = 0; r < E; ++r) P[(j + T * r) * SU + ln] = X[c][r];      // [k][p2]
+  }
+  group_sync(bar_id, NT);
+  // unpack the two real rows' half spectra; D: forward transform along x
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+    const int km = (N - ln) % N;
+    const bool odd = j & 1;
+#pragma unroll
+    for (int r = 0; r < E; ++r) {
+      const int p2 = (j + T * r) >> 1;
+      const float2 zk = P[ln * SU + p2], zm = P[km * SU + p2];
+      X[c][r] = odd ? make_float2(0.5f * (zk.y + zm.y), 0.5f * (zm.x - zk.x))
+                    : make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
+    }
+    fft_stage1<E, false>(X[c], w);
+  }
+  group_sync(bar_id, NT);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+#pragma unroll
+    for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[c][q];
+  }
+  group_sync(bar_id, NT);
+#pragma unroll
+  for (int c = 0; c < NC; ++c) {
+    float2* P = P0 + c * BUF;
+    fft_stage2<E, T, false>(X[c], j, [&](int q, int jj) { return P[(q * T + jj) * Y2 + ln]; });
+  }
+#pragma unroll
+  for (int r = 0; r < E; ++r) {
+    const int kx = j + T * r;
+    const float kap = s_kx[kx];
+    const size_t o = ((size_t)kx * nz + z) * Y2 + ln;
+    g.m0[o] = make_float2(-kap * X[0][r].y - kyv * X[1][r].y, kap * X[0][r].x + kyv * X[1][r].x);    // i kx J~x + i ky J~y
+    g.m2[o] = X[2][r];
+  }
+  group_sync(bar_id, NT);                       // the buffers are rewritten by the group's next unit
+}
+
 // shared memory of one z-line group (transient part).  `red` (partial pad-layer sums, written after the per-mode
 // update), `accp` (pad contributions, RES mode) and `cs` (charges times e^{-i kx x}, pass B) lie over `buf`
 // (exchange buffer of the transforms), which is dead whenever they are live.
@@ -627,7 +795,7 @@ template <int N, int EP, int NZ, int EZ, int TYL> struct PersistCfg {
   static constexpr int PG = kPersistThreads / PT, ZG = kPersistThreads / ZT;
   static_assert(PG >= 1 && ZG >= 1 && PG <= 8 && ZG <= 8, "group sizes");
   static constexpr bool MERGED = (N <= 64);                        // plane units carry the x and y components together
-  static constexpr size_t p_bytes = (size_t)PG * (MERGED ? 4 : 2) * PlaneCfg<N>::BUF * sizeof(float2);
+  static constexpr size_t p_bytes = (size_t)PG * (MERGED ? 3 : 2) * PlaneCfg<N>::BUF * sizeof(float2);
   static constexpr size_t z_bytes = (size_t)ZG * ZGroupSmem<NZ, EZ, TYL>::bytes;
   static constexpr size_t t_bytes = (size_t)kStageSlots * 3 * N * sizeof(float);
   static constexpr size_t phase_bytes = (p_bytes > z_bytes ? p_bytes : z_bytes) > t_bytes ? (p_bytes > z_bytes ? p_bytes : z_bytes) : t_bytes;
@@ -755,22 +923,18 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
     // units: nz "xy" units (components x and y of a plane together, twice the work) first, then nz "z" units
     const int grp = tid / PT, t = tid % PT;
     const int n_slots = n_cta * PG;
-    // the source of the group's NEXT unit is loaded before the current unit is transformed
-    float2 V[EP], Vn[EP];
     if constexpr (CF::MERGED) {
-      float2* P0 = reinterpret_cast<float2*>(phase) + (size_t)grp * 4 * PlaneCfg<N>::BUF;
-      int u = cta * PG + grp;
-      if (u < nz * 2) plane_load<N, EP>(V, u < nz ? srcV : srcE, nz, u < nz ? u : u - nz, t);
-      for (; u < nz * 2; u += n_slots) {
-        const int un = u + n_slots;
-        if (un < nz * 2) plane_load<N, EP>(Vn, un < nz ? srcV : srcE, nz, un < nz ? un : un - nz, t);
-        if (u < nz) plane_unit<N, EP, EMIT, 2>(g, nz, u, 0, V, P0, s_sdt, s_kxf, t, 1 + grp, slot);
-        else        plane_unit<N, EP, EMIT, 1>(g, nz, u - nz, 2, V, P0, s_sdt, s_kxf, t, 1 + grp, slot);
-#pragma unroll
-        for (int r = 0; r < EP; ++r) V[r] = Vn[r];
+      // one unit = all three components of a plane: nz units for n_cta * PG groups (a single round at configs[1])
+      float2 VV[EP], VE[EP];
+      float2* P0 = reinterpret_cast<float2*>(phase) + (size_t)grp * 3 * PlaneCfg<N>::BUF;
+      for (int u = cta * PG + grp; u < nz; u += n_slots) {
+        plane_load<N, EP>(VV, srcV, nz, u, t);
+        plane_load<N, EP>(VE, srcE, nz, u, t);
+        plane_unit3<N, EP, EMIT>(g, nz, u, VV, VE, P0, s_sdt, s_kxf, t, 1 + grp, slot);
       }
     } else {
       float2* P0 = reinterpret_cast<float2*>(phase) + (size_t)grp * 2 * PlaneCfg<N>::BUF;
+      float2 V[EP];
       for (int u = cta * PG + grp; u < nz * 3; u += n_slots) {
         const int z = u / 3, comp = u - 3 * z;
         plane_load<N, EP>(V, comp == 2 ? srcE : srcV, nz, z, t);
