@@ -353,6 +353,123 @@ def convolve_currents(H, shape, lengths, nt, dt, v_w, carrier_step_offsets, pos,
     return tr
 
 
+# ----------------------------------------------------------------------------------------
+# carrier transport in the solved field ("computing the paths of the carriers",
+# :101 "dominates the time-to-insight"; BASELINE.json configs[1]: saturated-drift model
+# v = mu E / (1 + mu E / v_sat), mu_e = 1800, mu_h = 1500 cm^2/Vs, v_sat = 1.5e7 cm/s, up to nt steps)
+# ----------------------------------------------------------------------------------------
+def static_field(H, dt):
+    """Es[node] = sum_n H[node][n] dt = -grad_s W[nt-1] (R2 telescoped): the static weighting field of the table,
+    per volt of V_w.  H: [nx,ny,nz,nt,3]; returns float64 [nx,ny,nz,3] (the library sums in fp32 pairs: compared
+    within fp32 rounding)."""
+    return np.asarray(H, dtype=np.float64).sum(axis=3) * float(dt)
+
+
+def drift_trajectories(es, desc, start, sign, v_bias, mu_e, mu_h, v_sat, max_steps):
+    """Explicit Euler transport on H's time grid, ALL arithmetic in float32 in the order written here (the library does
+    the same operations without FMA contraction, so that step counts -- decided by float comparisons -- and positions are
+    bit-exact; R35 of DESIGN.md):
+        E   = v_bias * trilinear(Es, x)            indices / fractions by trajectory_nodes (R24); weights w = (wx*wy)*wz;
+                                                   sum over the corners k = 4 cx + 2 cy + cz in that order, e += w * Es
+        |E| = sqrt((Ex*Ex + Ey*Ey) + Ez*Ez)
+        v   = ((sign * mu) * E) / (1 + (mu * |E|) / v_sat)          mu = mu_e for sign < 0 (electron), mu_h for sign > 0
+        x'  = x + v * dt ;   recorded pos[m] = x, vel[m] = (x' - x) / dt    (R22: velocity as inferred by the trajectory)
+    A carrier is alive at x iff 0 <= z <= lz and, for every column, the minimum-image lateral distance^2 to the axis
+    (fmod(|x - cx|, lx), min(d, lx - d), dx*dx + dy*dy) is > r*r; it records a step only while alive, at most max_steps.
+    es: [nx,ny,nz,3] (cast to float32); start [C,3]; sign [C] (-1 / +1).
+    Returns (carrier_step_offsets int64 [C+1], pos float32 [S,3], vel float32 [S,3])."""
+    f32 = np.float32
+    nx, ny, nz = desc["nx"], desc["ny"], desc["nz"]
+    shape, lengths = (nx, ny, nz), (desc["lx"], desc["ly"], desc["lz"])
+    E = np.asarray(es, dtype=f32).reshape(nx, ny, nz, 3)
+    lx, ly, lz, dt = f32(desc["lx"]), f32(desc["ly"]), f32(desc["lz"]), f32(desc["dt"])
+    cols = [(f32(c["cx"]), f32(c["cy"]), f32(f32(c["radius"]) * f32(c["radius"]))) for c in desc["columns"]]
+    vb, vs = f32(v_bias), f32(v_sat)
+    start = np.asarray(start, dtype=f32).reshape(-1, 3)
+    offs, pos, vel = [0], [], []
+
+    def alive(x):
+        if not (x[2] >= f32(0.0) and x[2] <= lz):
+            return False
+        for (cx, cy, r2) in cols:
+            dx = np.fmod(np.abs(f32(x[0] - cx)), lx)
+            dx = min(dx, f32(lx - dx))
+            dy = np.fmod(np.abs(f32(x[1] - cy)), ly)
+            dy = min(dy, f32(ly - dy))
+            if not (f32(f32(dx * dx) + f32(dy * dy)) > r2):
+                return False
+        return True
+
+    for c in range(len(start)):
+        x = start[c].copy()
+        mu = f32(mu_e) if sign[c] < 0 else f32(mu_h)
+        smu = f32(f32(sign[c]) * mu)
+        m = 0
+        while m < max_steps and np.isfinite(x).all() and alive(x):
+            i0, i1, f, _ = trajectory_nodes(shape, lengths, x[None, :])
+            e = np.zeros(3, dtype=f32)
+            for cx_ in (0, 1):
+                wx = f[0, 0] if cx_ else f32(f32(1.0) - f[0, 0])
+                for cy_ in (0, 1):
+                    wy = f[0, 1] if cy_ else f32(f32(1.0) - f[0, 1])
+                    for cz_ in (0, 1):
+                        wz = f[0, 2] if cz_ else f32(f32(1.0) - f[0, 2])
+                        w = f32(f32(wx * wy) * wz)
+                        node = E[(i1 if cx_ else i0)[0, 0], (i1 if cy_ else i0)[0, 1], (i1 if cz_ else i0)[0, 2]]
+                        e = (e + (w * node).astype(f32)).astype(f32)
+            e = (vb * e).astype(f32)
+            en = np.sqrt(f32(f32(f32(e[0] * e[0]) + f32(e[1] * e[1])) + f32(e[2] * e[2])))
+            den = f32(f32(1.0) + f32(f32(mu * en) / vs))
+            v = ((smu * e).astype(f32) / den).astype(f32)
+            xn = (x + (v * dt).astype(f32)).astype(f32)
+            pos.append(x.copy())
+            vel.append(((xn - x).astype(f32) / dt).astype(f32))
+            x = xn
+            m += 1
+        offs.append(offs[-1] + m)
+    return (np.asarray(offs, dtype=np.int64), np.asarray(pos, dtype=f32).reshape(-1, 3), np.asarray(vel, dtype=f32).reshape(-1, 3))
+
+
+# ----------------------------------------------------------------------------------------
+# SURVEY 8(f)-3: electronics stage (PAPER.md:75 "the induced signal is convolved with the transfer function of the
+# front-end electronics, and noise is added"): causal FIR on H's time grid + additive noise + constant-fraction time
+# ----------------------------------------------------------------------------------------
+def electronics(currents, transfer, dt, noise=None, cfd_fraction=0.3):
+    """out[t][n] = dt * sum_{j <= n, j < len(transfer)} transfer[j] * currents[t][n - j]  (+ noise[t][n]);
+    t_cfd[t] = time of the first crossing of cfd_fraction * (extremum of out[t], by absolute value) on the way to that
+    extremum, linearly interpolated between samples (n - 1, n), in units of dt; -1 if the row is identically zero.
+    Returns (out float64 [T,nt], t_cfd float64 [T])."""
+    cur = np.asarray(currents, dtype=np.float64)
+    h = np.asarray(transfer, dtype=np.float64)
+    T, nt = cur.shape
+    out = np.zeros((T, nt))
+    for t in range(T):
+        for n in range(nt):
+            acc = 0.0
+            for j in range(min(len(h), n + 1)):
+                acc += h[j] * cur[t, n - j]
+            out[t, n] = acc * float(dt)
+    if noise is not None:
+        out = out + np.asarray(noise, dtype=np.float64)
+    t_cfd = np.full(T, -1.0)
+    for t in range(T):
+        k = int(np.argmax(np.abs(out[t])))
+        peak = out[t, k]
+        if peak == 0.0:
+            continue
+        thr = cfd_fraction * peak
+        s = 1.0 if peak > 0 else -1.0
+        for n in range(k + 1):
+            if s * out[t, n] >= s * thr:
+                if n == 0:
+                    t_cfd[t] = 0.0
+                else:
+                    a, b = s * out[t, n - 1], s * out[t, n]
+                    t_cfd[t] = (n - 1) + (s * thr - a) / (b - a)
+                break
+    return out, t_cfd
+
+
 # error metrics (R27) ---------------------------------------------------------------------
 def h_rel_l2(h_test, h_ref) -> float:
     a = np.asarray(h_test, dtype=np.float64).ravel()
