@@ -107,6 +107,40 @@ int wt_convolve_currents(const wt_geometry* geom, const float* H_dev,
 /* Releases a handle returned by wt_make_geometry.  NULL is a no-op. */
 void wt_free(void* handle);
 
+/* ---- around the hot path ----------------------------- */
+
+/* Static weighting field of a table, per volt of v_w:  Es[node][a] = dt * sum_n H[node][n][a]  (= -grad_s W[nt-1], the
+ * telescoped response; R2).  es_dev: [nx*ny*nz][3] fp32 in the node order of the table. */
+int wt_static_field(const wt_geometry* geom, const float* H_dev, float* es_dev, void* cuda_stream);
+
+/* Carrier transport in the solved field (PAPER.md:73 "computing the paths of the carriers", :101; BASELINE.json
+ * configs[1] saturated-drift model), explicit Euler on H's time grid, fp32 in a fixed order (R35):
+ *   E = v_bias * trilinear(Es, x)  (indices and fractions as wt_trajectory_nodes);  v = sign mu E / (1 + mu |E| / v_sat),
+ *   mu = mu_e for sign < 0, mu_h for sign > 0;  x' = x + v dt;  recorded pos[m] = x, vel[m] = (x' - x)/dt  (R22).
+ * A carrier records steps while 0 <= z <= lz and it is outside every column radius (minimum image in x, y), at most
+ * max_steps.  Two calls, so that the caller can size the outputs (it reads offsets[n_carriers] in between):
+ *   wt_drift_count          counts_dev[c] = number of steps of carrier c
+ *   wt_offsets_from_counts  offsets_dev[0] = 0, offsets_dev[i+1] = counts[0] + ... + counts[i]   (CSR offsets of Eq. 1.1)
+ *   wt_drift_fill           pos_dev / vel_dev [offsets[n_carriers]][3] in the layout wt_convolve_currents reads
+ * start_dev [C][3] fp32 um, sign_dev [C] int8 (-1 electron, +1 hole); units um, ns, V (mu in um^2/(V ns), v_sat in um/ns).
+ * workspace: >= wt_drift_workspace_bytes, 256-byte aligned. */
+int wt_drift_workspace_bytes(const wt_geometry* geom, size_t* bytes);
+int wt_drift_count(const wt_geometry* geom, const float* es_dev, double v_bias, double mu_e, double mu_h, double v_sat,
+                   int64_t n_carriers, const float* start_dev, const int8_t* sign_dev, int max_steps, int64_t* counts_dev,
+                   void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+int wt_offsets_from_counts(int64_t n, const int64_t* counts_dev, int64_t* offsets_dev, void* cuda_stream);
+int wt_drift_fill(const wt_geometry* geom, const float* es_dev, double v_bias, double mu_e, double mu_h, double v_sat,
+                  int64_t n_carriers, const float* start_dev, const int8_t* sign_dev, int max_steps,
+                  const int64_t* carrier_step_offsets_dev, float* pos_dev, float* vel_dev,
+                  void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
+
+/* Electronics stage ("convolved with the transfer function of the front-end electronics, and noise is
+ * added"):  out[r][n] = dt * sum_{j <= n, j < n_transfer} transfer[j] * currents[r][n - j]  (+ noise[r][n] if noise_dev),
+ * t_cfd[r] = first crossing of cfd_fraction * (extremum of out[r] by absolute value) on the way to that extremum,
+ * linearly interpolated, in units of dt; -1 for an all-zero row.  All arrays fp32 on the device; rows of nt samples. */
+int wt_electronics(int64_t n_rows, int nt, const float* currents_dev, const float* transfer_dev, int n_transfer,
+                   const float* noise_dev, double dt, double cfd_fraction, float* out_dev, float* t_cfd_dev, void* cuda_stream);
+
 /* ---- helpers ------------------------------------------------------------------------------ */
 
 /* Step a9 on its own (R24), for bit-exact index checks:  per step s

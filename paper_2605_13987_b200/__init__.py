@@ -21,7 +21,8 @@ WT_Q_N_NODES, WT_Q_N_CONDUCTING, WT_Q_N_PAD_LAYERS, WT_Q_NT = 5, 6, 7, 8
 WT_A_COLUMN_ID, WT_A_PAD_NODES, WT_A_PAD_POTENTIAL, WT_A_AINV, WT_A_GT, WT_A_GZT = 1, 2, 3, 4, 5, 6
 
 EXPORTS = ("wt_make_geometry", "wt_solve_H", "wt_convolve_currents", "wt_free", "wt_trajectory_nodes",
-           "wt_conv_workspace_bytes", "wt_query", "wt_get_array", "wt_last_error", "wt_launch_count", "wt_describe_plan", "wt_measure_fp32_fma")
+           "wt_conv_workspace_bytes", "wt_query", "wt_get_array", "wt_last_error", "wt_launch_count", "wt_describe_plan", "wt_measure_fp32_fma", "wt_static_field",
+           "wt_drift_workspace_bytes", "wt_drift_count", "wt_offsets_from_counts", "wt_drift_fill", "wt_electronics")
 
 
 class wt_column(C.Structure):
@@ -67,6 +68,15 @@ def _load():
     lib.wt_describe_plan.restype = C.c_int
     lib.wt_measure_fp32_fma.argtypes = [vp, sz, vp, C.POINTER(C.c_double)]
     lib.wt_measure_fp32_fma.restype = C.c_int
+    dbl = C.c_double
+    lib.wt_static_field.argtypes = [vp, vp, vp, vp]
+    lib.wt_drift_workspace_bytes.argtypes = [vp, C.POINTER(sz)]
+    lib.wt_drift_count.argtypes = [vp, vp, dbl, dbl, dbl, dbl, i64, vp, vp, C.c_int, vp, vp, sz, vp]
+    lib.wt_offsets_from_counts.argtypes = [i64, vp, vp, vp]
+    lib.wt_drift_fill.argtypes = [vp, vp, dbl, dbl, dbl, dbl, i64, vp, vp, C.c_int, vp, vp, vp, vp, sz, vp]
+    lib.wt_electronics.argtypes = [i64, C.c_int, vp, vp, C.c_int, vp, dbl, dbl, vp, vp, vp]
+    for n in ("wt_static_field", "wt_drift_workspace_bytes", "wt_drift_count", "wt_offsets_from_counts", "wt_drift_fill", "wt_electronics"):
+        getattr(lib, n).restype = C.c_int
     lib.wt_last_error.restype = C.c_char_p
     lib.wt_launch_count.restype = C.c_int64
     for n in ("wt_make_geometry", "wt_solve_H", "wt_convolve_currents", "wt_trajectory_nodes",
@@ -235,6 +245,59 @@ def wt_describe_plan(geom: Geometry) -> str:
     buf = C.create_string_buffer(512)
     _check(_lib.wt_describe_plan(geom.handle, buf, len(buf)))
     return buf.value.decode()
+
+
+def wt_static_field(geom, H):
+    """Es = dt * sum_n H[..., n, :]: float32 [nx, ny, nz, 3] on H's device."""
+    import torch
+    nx, ny, nz = geom.shape
+    es = torch.empty((nx, ny, nz, 3), dtype=torch.float32, device=H.device)
+    _run_on_side_stream(H.device, lambda s: _lib.wt_static_field(geom.handle, H.data_ptr(), es.data_ptr(), s))
+    es.record_stream(_stream(H.device))
+    return es
+
+
+def wt_drift_carriers(geom, es, start, sign, v_bias, mu_e=180.0, mu_h=150.0, v_sat=150.0, max_steps=None):
+    """Saturated-drift transport of carriers in the static field `es` (wt_static_field).  start float32 [C,3], sign int8 [C]
+    on es's device.  Returns (carrier_step_offsets int64 [C+1], pos float32 [S,3], vel float32 [S,3]) on the device."""
+    import torch
+    dev = es.device
+    n = start.shape[0]
+    max_steps = geom.nt if max_steps is None else max_steps
+    assert start.dtype == torch.float32 and start.is_contiguous() and sign.dtype == torch.int8 and sign.is_contiguous()
+    need = C.c_size_t()
+    _check(_lib.wt_drift_workspace_bytes(geom.handle, C.byref(need)))
+    ws = torch.empty(need.value + 256, dtype=torch.uint8, device=dev)
+    wptr = (ws.data_ptr() + 255) // 256 * 256
+    counts = torch.empty(max(n, 1), dtype=torch.int64, device=dev)
+    offs = torch.empty(n + 1, dtype=torch.int64, device=dev)
+    args = (geom.handle, es.data_ptr(), float(v_bias), float(mu_e), float(mu_h), float(v_sat), n, start.data_ptr(), sign.data_ptr(), int(max_steps))
+    _run_on_side_stream(dev, lambda s: _lib.wt_drift_count(*args, counts.data_ptr(), wptr, need.value, s))
+    _run_on_side_stream(dev, lambda s: _lib.wt_offsets_from_counts(n, counts.data_ptr(), offs.data_ptr(), s))
+    total = int(offs[-1])                      # (the one host read: sizes of the outputs)
+    pos = torch.empty((total, 3), dtype=torch.float32, device=dev)
+    vel = torch.empty((total, 3), dtype=torch.float32, device=dev)
+    _run_on_side_stream(dev, lambda s: _lib.wt_drift_fill(*args, offs.data_ptr(), pos.data_ptr(), vel.data_ptr(), wptr, need.value, s))
+    for t in (ws, counts, offs, pos, vel):
+        t.record_stream(_stream(dev))
+    return offs, pos, vel
+
+
+def wt_electronics(currents, transfer, dt, noise=None, cfd_fraction=0.3):
+    """Front-end transfer function (causal FIR), optional additive noise, constant-fraction time per row.
+    Returns (out float32 [R, nt], t_cfd float32 [R])."""
+    import torch
+    dev = currents.device
+    rows, nt = currents.shape
+    assert currents.dtype == torch.float32 and currents.is_contiguous() and transfer.dtype == torch.float32 and transfer.is_contiguous()
+    out = torch.empty((rows, nt), dtype=torch.float32, device=dev)
+    tc = torch.empty(rows, dtype=torch.float32, device=dev)
+    nptr = noise.data_ptr() if noise is not None else 0
+    _run_on_side_stream(dev, lambda s: _lib.wt_electronics(rows, nt, currents.data_ptr(), transfer.data_ptr(), transfer.numel(), nptr, float(dt),
+                                                            float(cfd_fraction), out.data_ptr(), tc.data_ptr(), s))
+    for t in (out, tc):
+        t.record_stream(_stream(dev))
+    return out, tc
 
 
 def wt_measure_fp32_fma(device="cuda:0") -> float:

@@ -19,7 +19,8 @@ UNITS = {
     "csrc/solve.cu": HEADERS,
     "csrc/solve_chain.cu": HEADERS,
     "csrc/solve_persistent.cu": HEADERS,
-    "csrc/conv.cu": ["csrc/geometry.h", "../include/wtide.h"],
+    "csrc/conv.cu": ["csrc/geometry.h", "csrc/locate.cuh", "../include/wtide.h"],
+    "csrc/next.cu": ["csrc/geometry.h", "csrc/locate.cuh", "../include/wtide.h"],
     "csrc/static_field.cu": HEADERS,
     "csrc/peaks.cu": ["csrc/geometry.h", "../include/wtide.h"],
 }

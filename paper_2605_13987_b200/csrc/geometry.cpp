@@ -232,6 +232,7 @@ extern "C" int wt_make_geometry(const wt_geometry_desc* d, wt_geometry** out) {
     const wt_column& c = d->columns[j];
     const double sig = conductivity(c.resistivity);
     g->col_s[j] = sig / eps;
+    g->cols_f32.push_back((float)c.cx); g->cols_f32.push_back((float)c.cy); g->cols_f32.push_back((float)c.radius * (float)c.radius);
     sigma_max = std::max(sigma_max, sig);
     int kfirst = -1, klast = -1;
     for (int k = 0; k < nz; ++k)

@@ -21,6 +21,7 @@ struct wt_geometry {
   // setup results (host, fp64)
   std::vector<int8_t> col_id;       // [nx][ny][nz], -1 = diamond
   std::vector<double> col_s;        // per column: s = sigma/eps in 1/ns
+  std::vector<float> cols_f32;      // per column: (float)cx, (float)cy, (float)r * (float)r  (transport kernels, next.cu)
   std::vector<int32_t> pad_nodes;   // [B][3]
   std::vector<double> pad_pot;      // [B]
   std::vector<int32_t> layers;      // distinct pad z-layers
