@@ -348,13 +348,21 @@ def run_ours(args):
     ws_solve = torch.empty(K * wt.wt_query(g, wt.WT_Q_SOLVE_WORKSPACE_BYTES) + 256, dtype=torch.uint8, device=dev)
     wt.wt_solve_H(gs, H=H, workspace=ws_solve, device=dev)
     torch.cuda.synchronize()
-    e_static = H[0].view(n_nodes, nt, 3).sum(dim=1).mul_(d["dt"]).view(d["nx"], d["ny"], d["nz"], 3)
+    # trajectories: the library's own transport in the static field of the table just solved -- inputs of
+    # Eq. 1.1 made on the device, outside the timed region
+    from wtide_inputs.tracks import MU_E, MU_H, V_SAT, bias_voltage
+    t_gen0 = time.perf_counter()
+    e_static = wt.wt_static_field(g, H[0])
     theta_max = 15.0 if args.config == 4 else 10.0
     tracks = make_tracks(args.config, args.tracks * world, d, theta_max)[shard_tracks(args.tracks, world, rank)]
     start, sign, charge, toff = carriers_on_tracks(tracks, args.carriers, d)
-    csr = field_drift(e_static, d, start, sign, charge, toff)
+    c_off, c_pos, c_vel = wt.wt_drift_carriers(g, e_static, torch.as_tensor(start).to(dev), torch.as_tensor(sign).to(dev), bias_voltage(d),
+                                               MU_E, MU_H, V_SAT, max_steps=nt)
+    csr = {"track_carrier_offsets": torch.as_tensor(toff, dtype=torch.int64).to(dev), "carrier_step_offsets": c_off, "pos": c_pos, "vel": c_vel,
+           "charge": torch.as_tensor(charge).to(dev)}
     del e_static
     torch.cuda.synchronize()
+    trajectory_gen_s = time.perf_counter() - t_gen0
     off_host = csr["carrier_step_offsets"].cpu().numpy()
     terms = count_terms(off_host, nt)
     n_steps_total = int(off_host[-1])
@@ -523,7 +531,9 @@ def run_ours(args):
                         "max_dev_from_one_call_result_rel_peak": e2e_dev,
                         "h_solve_e2e_s": h_solve_e2e_s,
                         "h_solve_e2e_what": "descriptor -> wt_make_geometry -> wt_solve_H -> synchronize -> one table row on the host, wall clock"},
-                "gpu_launches": int(launches), "clocks": clk.summary(), "wall_s_timed_region": wall}
+                "gpu_launches": int(launches), "clocks": clk.summary(), "wall_s_timed_region": wall,
+                "inputs": {"trajectories": "wt_static_field + wt_drift_carriers (saturated drift in the solved field, on the device, outside the timed region)",
+                           "trajectory_generation_s": trajectory_gen_s}}
         if not args.no_cpu_baseline and world == 1:
             # the oracle on a bounded sample of the same workload (first carriers of track 0), rows of
             # the same fp32 table fetched once
@@ -567,8 +577,9 @@ def run_sweep(args, wt, dev, world, rank):
     import torch
     import torch.distributed as dist
 
-    from wtide_inputs import carriers_on_tracks, field_drift, make_tracks, reduced_desc
+    from wtide_inputs import carriers_on_tracks, make_tracks, reduced_desc
     from wtide_inputs.configs import sweep_descs
+    from wtide_inputs.tracks import MU_E, MU_H, V_SAT, bias_voltage
     descs = sweep_descs()
     if args.nt:
         descs = [reduced_desc(dd, nt=args.nt) for dd in descs]
@@ -605,10 +616,13 @@ def run_sweep(args, wt, dev, world, rank):
             e[1].record(side)
             torch.cuda.synchronize()
             # inputs of Eq. 1.1 (outside every timed quantity): drift in the static field of this table
-            e_static = H.view(n_nodes, nt, 3).sum(dim=1).mul_(dd["dt"]).view(dd["nx"], dd["ny"], dd["nz"], 3)
+            e_static = wt.wt_static_field(g, H)
             tracks = make_tracks(3, n_tracks, dd, 10.0)
             start, sign, charge, toff = carriers_on_tracks(tracks, args.carriers, dd)
-            csr = field_drift(e_static, dd, start, sign, charge, toff)
+            c_off, c_pos, c_vel = wt.wt_drift_carriers(g, e_static, torch.as_tensor(start).to(dev), torch.as_tensor(sign).to(dev), bias_voltage(dd),
+                                                       MU_E, MU_H, V_SAT, max_steps=nt)
+            csr = {"track_carrier_offsets": torch.as_tensor(toff, dtype=torch.int64).to(dev), "carrier_step_offsets": c_off, "pos": c_pos,
+                   "vel": c_vel, "charge": torch.as_tensor(charge).to(dev)}
             del e_static
             n_car = csr["carrier_step_offsets"].numel() - 1
             wsc = torch.empty(wt.wt_conv_workspace_bytes(g, n_tracks, n_car, True) + 256, dtype=torch.uint8, device=dev)

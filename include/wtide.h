@@ -40,6 +40,9 @@ extern "C" {
 
 #define WT_BIAS    0     /* pad held at 0 V                         */
 #define WT_READOUT 1     /* pad stepped to v_w at t = 0  (R2, R4)   */
+#define WT_SEGMENT 2     /* conductive cylinder WITHOUT a contact pad: segments stacked on a pad column (same axis, other
+                            z range, other resistivity) give a depth-dependent conductivity profile; where
+                            columns overlap the first in the list wins (R13) */
 
 typedef struct wt_geometry wt_geometry; /* opaque; created by wt_make_geometry, released by wt_free */
 
@@ -49,8 +52,8 @@ typedef struct {
   double radius;       /* um, > 0                                                                */
   double resistivity;  /* ohm*cm, > 0  (0.75 ohm cm for the test-beam sensor)      */
   double z0, z1;       /* depth extent, um, 0 <= z0 < z1 <= lz                                   */
-  int    role;         /* WT_BIAS or WT_READOUT                                                  */
-  int    pad_at_z1;    /* 0: the contact pad is the column's first z-layer, 1: its last (R8)     */
+  int    role;         /* WT_BIAS, WT_READOUT or WT_SEGMENT                                      */
+  int    pad_at_z1;    /* 0: the contact pad is the column's first z-layer, 1: its last (R8); ignored for segments */
 } wt_column;
 
 /* "a text file describing the geometry of the conductive elements" as a C struct. */

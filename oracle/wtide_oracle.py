@@ -35,6 +35,7 @@ import scipy.linalg
 EPS0 = 8.8541878128e-12 * 1e-6 / 1.602176634e-19
 WT_BIAS = 0
 WT_READOUT = 1
+WT_SEGMENT = 2       # conductive cylinder without a contact pad (stacked segments: depth-dependent conductivity)
 
 
 def conductivity(resistivity_ohm_cm: float) -> float:
@@ -78,7 +79,8 @@ def voxelize(desc: dict):
     A node belongs to column j iff its minimum-image lateral distance^2 to the axis is <= r^2
     and z0 <= z <= z1; the first column in the list wins on overlap.  Pad nodes of a column =
     its nodes in its first (pad_at_z1 = 0) or last (pad_at_z1 = 1) z-layer; V_pad = v_w for
-    readout columns, 0 for bias columns (R4, R8).  Pad order: column order, then (ix, iy) row-major.
+    readout columns, 0 for bias columns (R4, R8); WT_SEGMENT columns conduct but carry no pad.  Pad order: column
+    order, then (ix, iy) row-major.
     """
     nx, ny, nz = desc["nx"], desc["ny"], desc["nz"]
     lx, ly, lz = desc["lx"], desc["ly"], desc["lz"]
@@ -100,6 +102,8 @@ def voxelize(desc: dict):
         member = inxy[:, :, None] & inz[None, None, :] & (col_id < 0)
         col_id[member] = j
         sigma[member] = conductivity(col["resistivity"])
+        if col["role"] == WT_SEGMENT:
+            continue
         layers = np.nonzero(inz)[0]
         kpad = int(layers[-1] if col["pad_at_z1"] else layers[0])
         ij = np.argwhere(member[:, :, kpad])

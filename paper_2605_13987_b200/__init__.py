@@ -15,7 +15,7 @@ import numpy as np
 from . import build as _build
 
 WT_OK, WT_EINVAL, WT_EGEOM, WT_EUNSTABLE, WT_ENOMEM, WT_ECUDA = 0, -1, -2, -3, -4, -5
-WT_BIAS, WT_READOUT = 0, 1
+WT_BIAS, WT_READOUT, WT_SEGMENT = 0, 1, 2
 WT_Q_H_BYTES, WT_Q_SOLVE_WORKSPACE_BYTES, WT_Q_SUBSTEPS, WT_Q_N_PADS = 1, 2, 3, 4
 WT_Q_N_NODES, WT_Q_N_CONDUCTING, WT_Q_N_PAD_LAYERS, WT_Q_NT = 5, 6, 7, 8
 WT_A_COLUMN_ID, WT_A_PAD_NODES, WT_A_PAD_POTENTIAL, WT_A_AINV, WT_A_GT, WT_A_GZT = 1, 2, 3, 4, 5, 6

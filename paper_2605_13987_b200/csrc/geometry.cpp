@@ -205,7 +205,7 @@ extern "C" int wt_make_geometry(const wt_geometry_desc* d, wt_geometry** out) {
   for (int j = 0; j < d->n_columns; ++j) {
     const wt_column& c = d->columns[j];
     if (!(c.radius > 0 && c.resistivity > 0 && c.z0 >= 0 && c.z0 < c.z1 && c.z1 <= d->lz) ||
-        (c.role != WT_BIAS && c.role != WT_READOUT) || !std::isfinite(c.cx) || !std::isfinite(c.cy)) {
+        (c.role != WT_BIAS && c.role != WT_READOUT && c.role != WT_SEGMENT) || !std::isfinite(c.cx) || !std::isfinite(c.cy)) {
       wt_set_error("wt_make_geometry: bad column " + std::to_string(j)); return WT_EINVAL;
     }
     any_readout |= (c.role == WT_READOUT);
@@ -256,7 +256,7 @@ extern "C" int wt_make_geometry(const wt_geometry_desc* d, wt_geometry** out) {
           if (id >= 0) continue;
           id = (int8_t)j;
           ++g->n_conducting;
-          if (k == kpad) {
+          if (k == kpad && c.role != WT_SEGMENT) {
             g->pad_nodes.push_back(ix); g->pad_nodes.push_back(iy); g->pad_nodes.push_back(k);
             g->pad_pot.push_back(c.role == WT_READOUT ? d->v_w : 0.0);
             ++n_pad;
@@ -265,7 +265,7 @@ extern "C" int wt_make_geometry(const wt_geometry_desc* d, wt_geometry** out) {
       }
     }
     if (!any_xy) { delete g; wt_set_error("wt_make_geometry: column " + std::to_string(j) + " contains no grid node"); return WT_EGEOM; }
-    if (n_pad == 0) { delete g; wt_set_error("wt_make_geometry: column " + std::to_string(j) + " has no pad node"); return WT_EGEOM; }
+    if (n_pad == 0 && c.role != WT_SEGMENT) { delete g; wt_set_error("wt_make_geometry: column " + std::to_string(j) + " has no pad node"); return WT_EGEOM; }
   }
   const int B = (int)g->pad_pot.size();
 

@@ -237,3 +237,43 @@ def test_full_grid_window_matches_the_oracle(name, full_size_oracles):
     assert np.isfinite(h).all()
     assert err <= TOL, (name, err, per_slice)
     assert per_slice.max() <= 20 * TOL, (name, per_slice)
+
+
+def _segmented(desc, rhos=(2.0, 8.0)):
+    """the readout column of `desc` with its lower two thirds replaced by two segments of other resistivities"""
+    d = reduced_desc(desc)
+    ro = d["columns"][0]
+    z0, z1 = ro["z0"], ro["z1"]
+    a, b = z0 + (z1 - z0) / 3, z0 + 2 * (z1 - z0) / 3
+    d["columns"] = [dict(ro, z1=a), dict(ro, z0=a, z1=b, resistivity=rhos[0], role=wt.WT_SEGMENT),
+                    dict(ro, z0=b, resistivity=rhos[1], role=wt.WT_SEGMENT)] + d["columns"][1:]
+    return d
+
+
+@pytest.mark.parametrize("grid,nt", [((16, 16, 24), 4), ((32, 32, 64), 4), ((64, 64, 256), 4)])
+def test_depth_dependent_conductivity_profile(grid, nt):
+    """SURVEY 8(f) row 4 / PAPER.md:143: a column whose conductivity changes with depth (WT_SEGMENT stacks) through the
+    size-generic kernels, the register-FFT chain and the persistent kernel (full configs[1] grid), against the oracle."""
+    base = square_cell(55.0, 500.0 if grid[2] == 256 else 60.0, grid, nt, 0.005, 5.0, 1.0, 5.0, 1.0)
+    d = _segmented(base)
+    (g,), (h,) = _solve([d])
+    if grid == (64, 64, 256):
+        assert wt.wt_describe_plan(g).startswith("persistent")
+    ref = wo.solve_H_from_desc(d)
+    assert wo.h_rel_l2(h, ref) <= TOL
+    # and the profile matters: the table differs from the uniform column's by far more than the tolerance
+    _, (h0,) = _solve([base])
+    assert wo.h_rel_l2(h0, ref) > 50 * TOL
+
+
+def test_every_electrode_as_readout_in_one_lock_step_batch():
+    """SURVEY 8(f) row 4 'several readout electrodes solved at once': the geometries of a batch differ only in which
+    column is driven.  Each table matches the oracle, and the tables of all electrodes add up to zero (north_star
+    check 2, superposition of the weighting potentials over all electrodes)."""
+    d_a = square_cell(55.0, 50.0, (32, 32, 32), 8, 0.01, 5.0, 0.5, 4.0, 0.8)
+    d_b = reduced_desc(d_a)
+    d_b["columns"][0]["role"], d_b["columns"][1]["role"] = wt.WT_BIAS, wt.WT_READOUT
+    _, (ha, hb) = _solve([d_a, d_b])
+    for h, d in ((ha, d_a), (hb, d_b)):
+        assert wo.h_rel_l2(h, wo.solve_H_from_desc(d)) <= TOL
+    assert np.abs(ha.astype(np.float64) + hb).max() <= 1e-4 * np.abs(ha).max()

@@ -77,3 +77,26 @@ def test_error_codes():
     assert wt.wt_query(g, wt.WT_Q_SUBSTEPS) == 25
     with pytest.raises(wt.WtideError):
         wt.wt_query(g, 999)
+
+
+def test_segments_give_a_depth_dependent_profile_and_match_the_oracle_voxeliser():
+    """WT_SEGMENT (PAPER.md:143 'depth-dependent conductivity profile'): a readout column whose lower
+    part is a stack of two segments of other resistivities.  Same node sets and pads as the oracle's voxeliser, bit-exact;
+    a stack of segments with the SAME resistivity equals the single full-depth column."""
+    from wtide_inputs.configs import square_cell
+    base = square_cell(40.0, 60.0, (16, 16, 24), 8, 0.01, 5.0, 0.5, 5.0, 0.5)
+    ro = base["columns"][0]
+    seg = dict(base)
+    seg["columns"] = [dict(ro, z1=20.0), dict(ro, z0=20.0, z1=40.0, resistivity=2.0, role=wt.WT_SEGMENT), dict(ro, z0=40.0, resistivity=8.0, role=wt.WT_SEGMENT),
+                      base["columns"][1]]
+    g = wt.wt_make_geometry(seg)
+    col_id, sigma, pads, pot, pcol = wo.voxelize(seg)
+    assert np.array_equal(wt.wt_get_array(g, wt.WT_A_COLUMN_ID), col_id.astype(np.int8))
+    assert np.array_equal(wt.wt_get_array(g, wt.WT_A_PAD_NODES), pads.astype(np.int32))
+    assert set(pcol) == {0, 3} and (col_id == 1).any() and (col_id == 2).any()
+    assert wt.wt_query(g, wt.WT_Q_SUBSTEPS) == wo.substeps_from_desc(seg)
+    same = dict(base)
+    same["columns"] = [dict(ro, z1=20.0), dict(ro, z0=20.0, role=wt.WT_SEGMENT), base["columns"][1]]
+    _, s_same, p_same, _, _ = wo.voxelize(same)
+    _, s_base, p_base, _, _ = wo.voxelize(base)
+    assert np.array_equal(s_same, s_base) and np.array_equal(p_same, p_base)
