@@ -358,6 +358,43 @@ def convolve_currents(H, shape, lengths, nt, dt, v_w, carrier_step_offsets, pos,
 
 
 # ----------------------------------------------------------------------------------------
+# electrostatic field ("An iterative pseudo-spectral method ... is used to solve the Laplace
+# equation in the diamond sensor", :95 V <-> rho through the 3-D FFT and |k|^2, Fig. 2 :107)
+# ----------------------------------------------------------------------------------------
+def static_potential(desc, column_potentials):
+    """The Laplace problem the iteration of Fig. 2 converges to, written out as its plain definition (R37 of DESIGN.md):
+    every node of column j is held at column_potentials[j] (whole columns are ideal conductors), there is no charge
+    anywhere else, the box is periodic and neutral:
+        V(x) = c + sum_{s in S} q_s G(x - x_s),   V(x_s) = v_s for s in S,   sum_s q_s = 0,
+    S = all column nodes (voxelize), G = the tabulated fundamental solution of the same spectral Laplacian (R9).
+    Solved here by one dense least-squares solve; the library iterates (conjugate gradients on the same system).
+    Returns (V[nx,ny,nz], E[nx,ny,nz,3] = -grad_s V, q[nx,ny,nz] in e)."""
+    col_id, _, _, _, _ = voxelize(desc)
+    prob = problem_from_desc(desc)
+    shape = prob.shape
+    nodes = np.argwhere(col_id >= 0)
+    vals = np.asarray(column_potentials, dtype=np.float64)[col_id[col_id >= 0]]
+    nb = len(nodes)
+    a = np.zeros((nb + 1, nb + 1))
+    for i in range(nb):
+        dd = (nodes[i][None, :] - nodes) % np.array(shape)
+        a[i, :nb] = prob.green[dd[:, 0], dd[:, 1], dd[:, 2]]
+    scale = float(prob.green[0, 0, 0])          # border in the units of G (keeps the matrix well scaled); c = scale * last unknown
+    a[:nb, nb] = scale
+    a[nb, :nb] = scale
+    # (charge patterns that lie in the removed Nyquist planes, or deep inside a conductor, barely change V: the system is
+    #  consistent but can be singular -- a column that spans every z layer, say -- so the minimum-norm solution is taken;
+    #  V and E are unique, q is not)
+    sol = scipy.linalg.lstsq(a, np.concatenate([vals, [0.0]]), cond=1e-13)[0]
+    q = np.zeros(shape)
+    q[nodes[:, 0], nodes[:, 1], nodes[:, 2]] = sol[:-1]
+    v = prob.potential_of_charge(q) + scale * sol[-1]
+    g = prob.grad_s(v)
+    e = np.stack([-g[0], -g[1], -g[2]], axis=-1)
+    return v, e, q
+
+
+# ----------------------------------------------------------------------------------------
 # SURVEY 8(f)-2: carrier transport in the solved field (PAPER.md:73 "computing the paths of the carriers",
 # :101 "dominates the time-to-insight"; BASELINE.json configs[1]: saturated-drift model
 # v = mu E / (1 + mu E / v_sat), mu_e = 1800, mu_h = 1500 cm^2/Vs, v_sat = 1.5e7 cm/s, up to nt steps)

@@ -95,3 +95,61 @@ def test_electronics_is_a_causal_fir_plus_noise_with_a_cfd_time():
     o4, t4 = wo.electronics(-ramp, np.array([1.0]), 1.0, cfd_fraction=0.3)          # negative pulses: same time
     assert abs(t4[0] - 2.4) < 1e-12
     assert wo.electronics(np.zeros((1, 8)), h, 1.0)[1][0] == -1.0
+
+
+# ---- the electrostatic (Laplace) field ---------------------------------------------------------------
+def _cell(grid=(16, 16, 8)):
+    return square_cell(40.0, 30.0, grid, 8, 0.01, 4.0, 0.5, 4.0, 0.5)
+
+
+def test_static_potential_reproduces_the_electrode_values_and_is_neutral():
+    d = _cell()
+    col_id, _, _, _, _ = wo.voxelize(d)
+    v, e, q = wo.static_potential(d, [1.0, -2.0])
+    assert np.abs(v[col_id == 0] - 1.0).max() <= 1e-10 and np.abs(v[col_id == 1] + 2.0).max() <= 1e-10
+    assert abs(q.sum()) <= 1e-9 * np.abs(q).sum() and (q[col_id < 0] == 0).all()
+    # between the electrodes the potential stays between their values (up to the ringing of the spectral operator)
+    assert v.min() >= -2.0 - 0.3 and v.max() <= 1.0 + 0.3
+
+
+def test_static_potential_is_linear_and_constant_when_all_electrodes_agree():
+    d = _cell()
+    v1, e1, _ = wo.static_potential(d, [1.0, 0.0])
+    v2, e2, _ = wo.static_potential(d, [0.0, 1.0])
+    v3, e3, _ = wo.static_potential(d, [3.0, -0.5])
+    assert np.abs(3.0 * v1 - 0.5 * v2 - v3).max() <= 1e-9
+    assert np.abs(3.0 * e1 - 0.5 * e2 - e3).max() <= 1e-9
+    vc, ec, qc = wo.static_potential(d, [0.7, 0.7])
+    assert np.abs(vc - 0.7).max() <= 1e-9 and np.abs(ec).max() <= 1e-9
+    assert np.abs((v1 + v2) - 1.0).max() <= 1e-9          # north_star check 2 in its static form
+
+
+def test_static_potential_has_the_logarithmic_profile_of_a_line_charge_near_a_thin_column():
+    """A thin full-depth column in a z-invariant cell: between a few grid spacings and a fraction of the pitch the potential
+    falls like -(lambda / 2 pi eps) ln r (coaxial textbook profile), lambda = charge per unit length of the column."""
+    d = dict(lx=64.0, ly=64.0, lz=8.0, nx=64, ny=64, nz=4, nt=4, dt=0.01, eps_r=5.7, v_w=1.0, substeps=0, columns=[
+        dict(cx=32.0, cy=32.0, radius=0.4, resistivity=0.5, z0=0.0, z1=8.0, role=wo.WT_READOUT, pad_at_z1=0),
+        dict(cx=0.0, cy=0.0, radius=0.4, resistivity=0.5, z0=0.0, z1=8.0, role=wo.WT_BIAS, pad_at_z1=0)])
+    v, e, q = wo.static_potential(d, [1.0, 0.0])
+    assert np.abs(v - v[:, :, :1]).max() <= 1e-9                                   # z-invariant
+    lam = q[32, 32, :].sum() / d["lz"]                                             # e per um
+    eps = d["eps_r"] * wo.EPS0
+    r1, r2 = 4, 10
+    slope = (v[32 + r2, 32, 0] - v[32 + r1, 32, 0]) / math.log(r2 / r1)
+    assert abs(slope / (-lam / (2 * math.pi * eps)) - 1.0) <= 0.05
+    # and the radial field there is lambda / (2 pi eps r).  The spectral gradient of the potential of a one-node-wide charge
+    # carries a two-node saw-tooth (the Nyquist plane is removed, R11/R14: part of the defined result), so the field is
+    # compared after the (1/4, 1/2, 1/4) average over neighbouring nodes that removes that component
+    ex = e[:, 32, 0, 0]
+    smooth = 0.25 * ex[32 + 5] + 0.5 * ex[32 + 6] + 0.25 * ex[32 + 7]
+    assert abs(smooth / (lam / (2 * math.pi * eps * 6.0)) - 1.0) <= 0.05
+    assert abs(-(v[32 + 7, 32, 0] - v[32 + 5, 32, 0]) / 2.0 / (lam / (2 * math.pi * eps * 6.0)) - 1.0) <= 0.03    # central difference of V
+
+
+def test_static_potential_equals_the_stationary_state_on_the_columns():
+    """The quasi-static solver's stationary state (tests/test_oracle_solve.py) and the Laplace solution hold the same
+    Dirichlet data: both put every column node at its electrode's potential."""
+    d = _cell((12, 12, 6))
+    col_id, _, _, _, _ = wo.voxelize(d)
+    v, _, _ = wo.static_potential(d, [d["v_w"], 0.0])
+    assert np.abs(v[col_id == 0] - d["v_w"]).max() <= 1e-10 and np.abs(v[col_id == 1]).max() <= 1e-10
