@@ -116,6 +116,29 @@ void wt_free(void* handle);
  * telescoped response; R2).  es_dev: [nx*ny*nz][3] fp32 in the node order of the table. */
 int wt_static_field(const wt_geometry* geom, const float* H_dev, float* es_dev, void* cuda_stream);
 
+/* the electrostatic field of the sensor ("An iterative pseudo-spectral method ... is used
+ * to solve the Laplace equation in the diamond sensor"; :95 V <-> rho by the 3-D FFT and a kernel that multiplies or divides by |k|^2;
+ * Fig. 2 :107).  Reading R37: every node of column j (the voxel set of wt_make_geometry, all roles) is held at column_potentials[j],
+ * there is no charge elsewhere, the box is periodic and neutral:  V(x) = c + sum_{s in S} q_s G(x - x_s), V = v_j on column j,
+ * sum q = 0, G = fundamental solution of the spectral Laplacian with the Nyquist modes removed (R9, R11).  Solved by conjugate
+ * gradients on the restricted operator in the neutral subspace, each step one V <-> rho round trip (forward 3-D DFT, times 1/|k|^2
+ * or |k|^2, inverse 3-D DFT, restriction to the electrodes), the whole iteration in ONE cooperative kernel launch.
+ *   column_potentials  HOST array [n_potentials], n_potentials = number of columns of the descriptor, volts
+ *   precondition       0: plain CG;  1: preconditioned by the restricted Laplacian (the rho-from-V direction of Fig. 2)
+ *   max_iter, tol      stop after max_iter steps or when |residual on the electrodes|_2 <= tol * |Pi v|_2
+ *   V_dev              [nx][ny][nz] fp32 (node order of the H table), may be NULL
+ *   E_dev              [nx*ny*nz][3] fp32 = -grad_s V in V/um, the layout wt_static_field writes (feeds wt_drift_* with
+ *                      v_bias = 1), may be NULL (not both)
+ *   info_dev           [4] fp64 on the device: iterations done (-1: the kernel gave up waiting for a lost CTA and the outputs
+ *                      are not valid), |residual|_2/|Pi v|_2, the constant c, sum of the charges (library units)
+ *   workspace          >= wt_static_workspace_bytes (41 bytes per node), 256-byte aligned
+ * q is not unique (R37), V and E are.  Transforms in fp32, CG vectors and sums in fp64; run-to-run deterministic.
+ * WT_EINVAL if an xy-plane of the grid does not fit in shared memory (nx*ny beyond about 24 000). */
+int wt_static_workspace_bytes(const wt_geometry* geom, size_t* bytes);
+int wt_solve_static(const wt_geometry* geom, const double* column_potentials, int n_potentials, int precondition, int max_iter,
+                    double tol, float* V_dev, float* E_dev, double* info_dev, void* workspace_dev, size_t workspace_bytes,
+                    void* cuda_stream);
+
 /* Carrier transport in the solved field (PAPER.md:73 "computing the paths of the carriers", :101; BASELINE.json
  * configs[1] saturated-drift model), explicit Euler on H's time grid, fp32 in a fixed order (R35):
  *   E = v_bias * trilinear(Es, x)  (indices and fractions as wt_trajectory_nodes);  v = sign mu E / (1 + mu |E| / v_sat),

@@ -22,7 +22,7 @@ WT_A_COLUMN_ID, WT_A_PAD_NODES, WT_A_PAD_POTENTIAL, WT_A_AINV, WT_A_GT, WT_A_GZT
 
 EXPORTS = ("wt_make_geometry", "wt_solve_H", "wt_convolve_currents", "wt_free", "wt_trajectory_nodes",
            "wt_conv_workspace_bytes", "wt_query", "wt_get_array", "wt_last_error", "wt_launch_count", "wt_describe_plan", "wt_measure_fp32_fma", "wt_static_field",
-           "wt_drift_workspace_bytes", "wt_drift_count", "wt_offsets_from_counts", "wt_drift_fill", "wt_electronics")
+           "wt_drift_workspace_bytes", "wt_drift_count", "wt_offsets_from_counts", "wt_drift_fill", "wt_electronics", "wt_static_workspace_bytes", "wt_solve_static")
 
 
 class wt_column(C.Structure):
@@ -75,7 +75,11 @@ def _load():
     lib.wt_offsets_from_counts.argtypes = [i64, vp, vp, vp]
     lib.wt_drift_fill.argtypes = [vp, vp, dbl, dbl, dbl, dbl, i64, vp, vp, C.c_int, vp, vp, vp, vp, sz, vp]
     lib.wt_electronics.argtypes = [i64, C.c_int, vp, vp, C.c_int, vp, dbl, dbl, vp, vp, vp]
-    for n in ("wt_static_field", "wt_drift_workspace_bytes", "wt_drift_count", "wt_offsets_from_counts", "wt_drift_fill", "wt_electronics"):
+    lib.wt_static_workspace_bytes.argtypes = [vp, C.POINTER(sz)]
+    lib.wt_solve_static.argtypes = [vp, C.POINTER(dbl), C.c_int, C.c_int, C.c_int, dbl, vp, vp, vp, vp, sz, vp]
+    lib.wt_static_workspace_bytes.restype = C.c_int
+    lib.wt_solve_static.restype = C.c_int
+    for n in ("wt_static_field", "wt_drift_workspace_bytes", "wt_drift_count", "wt_offsets_from_counts", "wt_drift_fill", "wt_electronics", "wt_static_workspace_bytes", "wt_solve_static"):
         getattr(lib, n).restype = C.c_int
     lib.wt_last_error.restype = C.c_char_p
     lib.wt_launch_count.restype = C.c_int64
@@ -255,6 +259,29 @@ def wt_static_field(geom, H):
     _run_on_side_stream(H.device, lambda s: _lib.wt_static_field(geom.handle, H.data_ptr(), es.data_ptr(), s))
     es.record_stream(_stream(H.device))
     return es
+
+
+def wt_solve_static(geom, column_potentials, precondition=True, max_iter=2000, tol=1e-7, want_v=True, want_e=True, device="cuda:0"):
+    """Electrostatic potential and field with whole columns as electrodes.
+    Returns (V float32 [nx,ny,nz] or None, E float32 [nx,ny,nz,3] or None, info float64 [4] on the device:
+    iterations, relative residual, constant c, sum of the charges)."""
+    import torch
+    nx, ny, nz = geom.shape
+    need = C.c_size_t()
+    _check(_lib.wt_static_workspace_bytes(geom.handle, C.byref(need)))
+    ws = torch.empty(need.value + 256, dtype=torch.uint8, device=device)
+    wptr = (ws.data_ptr() + 255) // 256 * 256
+    v = torch.empty((nx, ny, nz), dtype=torch.float32, device=device) if want_v else None
+    e = torch.empty((nx, ny, nz, 3), dtype=torch.float32, device=device) if want_e else None
+    info = torch.empty(4, dtype=torch.float64, device=device)
+    pots = (C.c_double * len(column_potentials))(*[float(x) for x in column_potentials])
+    _run_on_side_stream(device, lambda s: _lib.wt_solve_static(
+        geom.handle, pots, len(column_potentials), int(bool(precondition)), int(max_iter), float(tol),
+        v.data_ptr() if want_v else 0, e.data_ptr() if want_e else 0, info.data_ptr(), wptr, need.value, s))
+    for t in (ws, v, e, info):
+        if t is not None:
+            t.record_stream(_stream(device))
+    return v, e, info
 
 
 def wt_drift_carriers(geom, es, start, sign, v_bias, mu_e=180.0, mu_h=150.0, v_sat=150.0, max_steps=None):
