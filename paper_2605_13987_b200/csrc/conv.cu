@@ -131,7 +131,10 @@ struct SysParams {
 
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
-__global__ void __launch_bounds__(256, 2) k_conv_systolic(SysParams sp) {
+// CACHE: the 8 x 12 floats a lane owns of the current cell's rows stay in registers while the carrier stays in the cell
+// (a carrier of configs[2] / [4] spends 2-4 steps per cell: those steps are pure FMA + shuffle, no row is read again).
+template <bool CACHE>
+__global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams sp) {
   const ConvParams& p = sp.c;
   const int nt = p.nt, F = 3 * nt;
   const int tid = threadIdx.x, w = tid >> 5, t = tid & 31, nw = blockDim.x >> 5;
@@ -232,6 +235,8 @@ __global__ void __launch_bounds__(256, 2) k_conv_systolic(SysParams sp) {
       D[2][0] = fmaf(q1, h2.x, D[2][0]); D[2][1] = fmaf(q2, h2.y, D[2][1]); D[2][2] = fmaf(q0, h2.z, D[2][2]); D[2][3] = fmaf(q1, h2.w, D[2][3]);
     };
     const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 HC[CACHE ? 8 : 1][3];
+    unsigned long long cell_key = ~0ULL;             // (per carrier: the first step always loads)
 
     {
       for (int m0 = 0; m0 < M; m0 += kStepChunk) {
@@ -256,12 +261,27 @@ __global__ void __launch_bounds__(256, 2) k_conv_systolic(SysParams sp) {
         for (int jm = 0; jm < mc; ++jm) {
           const int m = m0 + jm;
           if (128 * w + m >= nt) break;              // every output of this warp is past nt from here on (warp uniform)
+          if constexpr (CACHE) {
+            // the cell is identified by the nodes of its corners 0 and 7 (a skipped step has both 0: never a real cell)
+            const unsigned long long key = ((unsigned long long)__float_as_uint(tab[jm * 8].x) << 32) | __float_as_uint(tab[jm * 8 + 7].x);
+            if (key != cell_key) {                   // (warp uniform)
+              cell_key = key;
 #pragma unroll
-          for (int k = 0; k < 8; ++k) {
-            const float4 e = tab[jm * 8 + k];
-            const float* __restrict__ src = p.H + (size_t)__float_as_uint(e.x) * F + f0;
-            const float4 h0 = v0 ? ldg4(src) : z4, h1 = v1 ? ldg4(src + 128) : z4, h2 = v2 ? ldg4(src + 256) : z4;
-            fma12(A, e, h0, h1, h2);
+              for (int k = 0; k < 8; ++k) {
+                const float* __restrict__ src = p.H + (size_t)__float_as_uint(tab[jm * 8 + k].x) * F + f0;
+                HC[k][0] = v0 ? ldg4(src) : z4; HC[k][1] = v1 ? ldg4(src + 128) : z4; HC[k][2] = v2 ? ldg4(src + 256) : z4;
+              }
+            }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) fma12(A, tab[jm * 8 + k], HC[k][0], HC[k][1], HC[k][2]);
+          } else {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) {
+              const float4 e = tab[jm * 8 + k];
+              const float* __restrict__ src = p.H + (size_t)__float_as_uint(e.x) * F + f0;
+              const float4 h0 = v0 ? ldg4(src) : z4, h1 = v1 ? ldg4(src + 128) : z4, h2 = v2 ? ldg4(src + 256) : z4;
+              fma12(A, e, h0, h1, h2);
+            }
           }
           shift(m);
         }
@@ -384,7 +404,11 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
     sp.c = p; sp.track_off = per_track ? track_carrier_offsets_dev : nullptr;
     sp.n_tracks = n_tracks; sp.n_carriers = n_carriers; sp.gc = gc; sp.stride = stride; sp.per_track = per_track ? 1 : 0;
     const size_t smem = (size_t)kStepChunk * 8 * sizeof(float4) + (size_t)nw * 3 * g->nt * sizeof(float);
-    auto fn = k_conv_systolic;
+    // rows cached in registers across the steps a carrier spends in one cell: pays when carriers take several steps per cell
+    // (fine time grids: nt >= 1024 in the BASELINE configs); WTIDE_CONV_CACHE=0/1 forces either kernel (both parity-tested)
+    bool cache = g->nt >= 1024;
+    if (const char* ev = std::getenv("WTIDE_CONV_CACHE")) cache = ev[0] == '1';
+    auto fn = cache ? k_conv_systolic<true> : k_conv_systolic<false>;
     cudaError_t ea = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (ea != cudaSuccess) { wt_set_error(std::string("wt_convolve_currents: ") + cudaGetErrorString(ea)); return WT_ECUDA; }
     ++g_wt_launches;

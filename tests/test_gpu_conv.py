@@ -231,3 +231,43 @@ def test_tables_beyond_2_31_floats_sampled_tracks(config):
         assert l2 <= TOL and mx <= 5 * TOL, (config, per_track, l2, mx)
     del H
     torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("cache", ["0", "1"])
+def test_row_cache_kernel_and_plain_kernel_agree_with_the_oracle(cache, monkeypatch):
+    """k_conv_systolic<CACHE> keeps the rows of the current cell in registers while a carrier stays in it; both kernels
+    (WTIDE_CONV_CACHE=0/1) on slow carriers that spend several steps per cell, stationary carriers, a skipped (non-finite)
+    step followed by steps in the cell at node (0, 0, 0), and cell changes across the periodic wrap and the z clamp."""
+    monkeypatch.setenv("WTIDE_CONV_CACHE", cache)
+    for nt in (128, 1024, 36):
+        d = reduced_desc(geometry_desc(0), grid=(12, 8, 6), nt=nt)
+        g = wt.wt_make_geometry(d)
+        rng = np.random.default_rng(100 + nt)
+        Hnp = rng.standard_normal((12, 8, 6, nt, 3)).astype(np.float32)
+        H = torch.as_tensor(Hnp).to(DEV)
+        cell = np.array([d["lx"] / 12, d["ly"] / 8, d["lz"] / 6])
+        lens = [60, 90, 33, 50, 1, 70]
+        off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+        pos = []
+        for c, n in enumerate(lens):
+            x0 = rng.uniform(0, 1, 3) * np.array([d["lx"], d["ly"], d["lz"]])
+            step = rng.normal(0, 0.15, size=(n, 3)) * cell           # several steps per cell
+            if c == 1:
+                step[:] = 0.0                                        # stationary carrier
+            if c == 2:
+                x0 = np.array([d["lx"] - 0.2 * cell[0], 0.1 * cell[1], d["lz"] - 0.3 * cell[2]])   # wraps in x, y; clamps in z
+                step = np.abs(step) * np.array([1, -1, 1])
+            pos.append(x0 + np.cumsum(step, axis=0))
+        pos = np.concatenate(pos).astype(np.float32)
+        # carrier 3: a non-finite step, then steps inside the cell whose corner 0 is node (0, 0, 0)
+        a = off[3]
+        pos[a] = [np.nan, 1.0, 1.0]
+        pos[a + 1:a + 6] = (rng.uniform(0.1, 0.9, size=(5, 3)) * cell).astype(np.float32)
+        vel = rng.standard_normal((int(off[-1]), 3)).astype(np.float32)
+        csr = dict(track_carrier_offsets=np.array([0, 2, 6], np.int64), carrier_step_offsets=off, pos=pos, vel=vel,
+                   charge=rng.standard_normal(len(lens)).astype(np.float32))
+        for per_track in (False, True):
+            got = _run(g, H, csr, per_track)
+            ref = _oracle(d, Hnp, csr, per_track)
+            assert np.isfinite(got).all()
+            assert np.abs(got - ref).max() <= TOL * np.abs(ref).max(), (nt, per_track)
