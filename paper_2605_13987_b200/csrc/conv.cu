@@ -132,7 +132,9 @@ struct SysParams {
 __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 
 // CACHE: the 8 x 12 floats a lane owns of the current cell's rows stay in registers while the carrier stays in the cell
-// (a carrier of configs[2] / [4] spends 2-4 steps per cell: those steps are pure FMA + shuffle, no row is read again).
+// (a carrier of configs[2] / [4] spends 2-4 steps per cell: those steps are pure FMA + shuffle, no row is read again); the
+// step table then holds (node, w * scale) pairs, the velocity and a cell key per step, and the three weights of a corner are
+// formed from the lane's rotated velocity by three multiplies.
 template <bool CACHE>
 __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams sp) {
   const ConvParams& p = sp.c;
@@ -143,6 +145,10 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
   float* P = reinterpret_cast<float*>(smraw + kStepChunk * 8 * sizeof(float4));   // [nw][F]
   float* Pw = P + (size_t)w * F;
   __shared__ int64_t s_track;
+  // CACHE: the step table holds (node, w * scale) pairs, the velocity and the cell key of each step instead of 8 x (node, c_x, c_y, c_z)
+  float2* tabc = reinterpret_cast<float2*>(smraw);                                // [kStepChunk][8]
+  float4* tabv = reinterpret_cast<float4*>(smraw + kStepChunk * 8 * sizeof(float2));          // [kStepChunk]
+  unsigned long long* keys = reinterpret_cast<unsigned long long*>(smraw + kStepChunk * (8 * sizeof(float2) + sizeof(float4)));   // [kStepChunk]
 
   const int f0 = 384 * w + 4 * t;
   const bool v0 = f0 < F, v1 = f0 + 128 < F, v2 = f0 + 256 < F;       // F % 4 == 0: whole 16-byte groups
@@ -234,6 +240,11 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
       D[1][0] = fmaf(q2, h1.x, D[1][0]); D[1][1] = fmaf(q0, h1.y, D[1][1]); D[1][2] = fmaf(q1, h1.z, D[1][2]); D[1][3] = fmaf(q2, h1.w, D[1][3]);
       D[2][0] = fmaf(q1, h2.x, D[2][0]); D[2][1] = fmaf(q2, h2.y, D[2][1]); D[2][2] = fmaf(q0, h2.z, D[2][2]); D[2][3] = fmaf(q1, h2.w, D[2][3]);
     };
+    auto fma12q = [&](float (&D)[3][4], const float q0, const float q1, const float q2, const float4 h0, const float4 h1, const float4 h2) {
+      D[0][0] = fmaf(q0, h0.x, D[0][0]); D[0][1] = fmaf(q1, h0.y, D[0][1]); D[0][2] = fmaf(q2, h0.z, D[0][2]); D[0][3] = fmaf(q0, h0.w, D[0][3]);
+      D[1][0] = fmaf(q2, h1.x, D[1][0]); D[1][1] = fmaf(q0, h1.y, D[1][1]); D[1][2] = fmaf(q1, h1.z, D[1][2]); D[1][3] = fmaf(q2, h1.w, D[1][3]);
+      D[2][0] = fmaf(q1, h2.x, D[2][0]); D[2][1] = fmaf(q2, h2.y, D[2][1]); D[2][2] = fmaf(q0, h2.z, D[2][2]); D[2][3] = fmaf(q1, h2.w, D[2][3]);
+    };
     const float4 z4 = make_float4(0.f, 0.f, 0.f, 0.f);
     float4 HC[CACHE ? 8 : 1][3];
     unsigned long long cell_key = ~0ULL;             // (per carrier: the first step always loads)
@@ -247,6 +258,7 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
           const float vx = p.vel[3 * s], vy = p.vel[3 * s + 1], vz = p.vel[3 * s + 2];
           const NodeFrac nf = locate(p.pos[3 * s], p.pos[3 * s + 1], p.pos[3 * s + 2], p.nx, p.ny, p.nz, p.invx, p.invy, p.invz);
           const bool ok = nf.ok && isfinite(vx) && isfinite(vy) && isfinite(vz);
+          unsigned key_hi = 0;
 #pragma unroll
           for (int k = 0; k < 8; ++k) {
             const int cx = k >> 2, cy = (k >> 1) & 1, cz = k & 1;
@@ -254,26 +266,41 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
             const int ix = cx ? nf.i1[0] : nf.i0[0], iy = cy ? nf.i1[1] : nf.i0[1], iz = cz ? nf.i1[2] : nf.i0[2];
             const unsigned node = ok ? (unsigned)((ix * p.ny + iy) * p.nz + iz) : 0u;
             const float ws = wgt * scale;            // a non-finite step contributes nothing (0, not 0 * inf)
-            tab[tid * 8 + k] = make_float4(__uint_as_float(node), ok ? ws * vx : 0.f, ok ? ws * vy : 0.f, ok ? ws * vz : 0.f);
+            if constexpr (CACHE) {
+              tabc[tid * 8 + k] = make_float2(__uint_as_float(node), ok ? ws : 0.f);
+              if (k == 0) key_hi = node;
+              if (k == 7) keys[tid] = ((unsigned long long)key_hi << 32) | node;   // corners 0 and 7 identify the cell (a skipped step has both 0: never a real cell)
+            } else {
+              tab[tid * 8 + k] = make_float4(__uint_as_float(node), ok ? ws * vx : 0.f, ok ? ws * vy : 0.f, ok ? ws * vz : 0.f);
+            }
           }
+          if constexpr (CACHE) tabv[tid] = ok ? make_float4(vx, vy, vz, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
         __syncthreads();
         for (int jm = 0; jm < mc; ++jm) {
           const int m = m0 + jm;
           if (128 * w + m >= nt) break;              // every output of this warp is past nt from here on (warp uniform)
           if constexpr (CACHE) {
-            // the cell is identified by the nodes of its corners 0 and 7 (a skipped step has both 0: never a real cell)
-            const unsigned long long key = ((unsigned long long)__float_as_uint(tab[jm * 8].x) << 32) | __float_as_uint(tab[jm * 8 + 7].x);
+            const unsigned long long key = keys[jm];
             if (key != cell_key) {                   // (warp uniform)
               cell_key = key;
 #pragma unroll
               for (int k = 0; k < 8; ++k) {
-                const float* __restrict__ src = p.H + (size_t)__float_as_uint(tab[jm * 8 + k].x) * F + f0;
+                const float* __restrict__ src = p.H + (size_t)__float_as_uint(tabc[jm * 8 + k].x) * F + f0;
                 HC[k][0] = v0 ? ldg4(src) : z4; HC[k][1] = v1 ? ldg4(src + 128) : z4; HC[k][2] = v2 ? ldg4(src + 256) : z4;
               }
             }
+            const float4 vv = tabv[jm];
+            const float q0 = r0 ? vv.x : (r1 ? vv.y : vv.z);      // velocity component (t + x) % 3, x = 0, 1, 2
+            const float q1 = r0 ? vv.y : (r1 ? vv.z : vv.x);
+            const float q2 = r0 ? vv.z : (r1 ? vv.x : vv.y);
+            const float4* tc4 = reinterpret_cast<const float4*>(tabc + jm * 8);
 #pragma unroll
-            for (int k = 0; k < 8; ++k) fma12(A, tab[jm * 8 + k], HC[k][0], HC[k][1], HC[k][2]);
+            for (int kk = 0; kk < 4; ++kk) {
+              const float4 e2 = tc4[kk];             // (node, w * scale) of corners 2 kk and 2 kk + 1
+              fma12q(A, e2.y * q0, e2.y * q1, e2.y * q2, HC[2 * kk][0], HC[2 * kk][1], HC[2 * kk][2]);
+              fma12q(A, e2.w * q0, e2.w * q1, e2.w * q2, HC[2 * kk + 1][0], HC[2 * kk + 1][1], HC[2 * kk + 1][2]);
+            }
           } else {
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
@@ -403,12 +430,12 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
     SysParams sp;
     sp.c = p; sp.track_off = per_track ? track_carrier_offsets_dev : nullptr;
     sp.n_tracks = n_tracks; sp.n_carriers = n_carriers; sp.gc = gc; sp.stride = stride; sp.per_track = per_track ? 1 : 0;
-    const size_t smem = (size_t)kStepChunk * 8 * sizeof(float4) + (size_t)nw * 3 * g->nt * sizeof(float);
     // rows cached in registers across the steps a carrier spends in one cell: pays when carriers take several steps per cell
     // (fine time grids: nt >= 1024 in the BASELINE configs); WTIDE_CONV_CACHE=0/1 forces either kernel (both parity-tested)
     bool cache = g->nt >= 1024;
     if (const char* ev = std::getenv("WTIDE_CONV_CACHE")) cache = ev[0] == '1';
     auto fn = cache ? k_conv_systolic<true> : k_conv_systolic<false>;
+    const size_t smem = (size_t)kStepChunk * 8 * sizeof(float4) + (size_t)nw * 3 * g->nt * sizeof(float);
     cudaError_t ea = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (ea != cudaSuccess) { wt_set_error(std::string("wt_convolve_currents: ") + cudaGetErrorString(ea)); return WT_ECUDA; }
     ++g_wt_launches;
