@@ -107,7 +107,7 @@ class Geometry:
 
     def __del__(self):
         h, self.handle = getattr(self, "handle", None), None
-        if h:
+        if h and _lib is not None:       # (module globals may already be gone at interpreter shutdown)
             _lib.wt_free(h)
 
     @property

@@ -102,13 +102,70 @@ __device__ __forceinline__ void dft16(float2 (&v)[16]) {
   t = v[11]; v[11] = v[14]; v[14] = t;
 }
 
+// ---- radix 3 (grids 96 = 2^5 3, 384 = 2^7 3 of BASELINE configs[4]) -------------------------------------------
+// a * e^{-+ 2 pi i K/24}  (forward: minus, inverse: plus), K compile-time
+template <int K, bool INV>
+__device__ __forceinline__ float2 mul_w24(float2 a) {
+  constexpr int k = ((K % 24) + 24) % 24;
+  constexpr float C1 = 0.96592582628906829f, C2 = 0.86602540378443865f, C3 = 0.70710678118654752f, C4 = 0.5f, C5 = 0.25881904510252076f;
+  // cos(2 pi k/24), sin(2 pi k/24), k = 0 .. 23 (steps of 15 degrees)
+  constexpr float cs[24] = {1.f, C1, C2, C3, C4, C5, 0.f, -C5, -C4, -C3, -C2, -C1, -1.f, -C1, -C2, -C3, -C4, -C5, 0.f, C5, C4, C3, C2, C1};
+  constexpr float sn[24] = {0.f, C5, C4, C3, C2, C1, 1.f, C1, C2, C3, C4, C5, 0.f, -C5, -C4, -C3, -C2, -C1, -1.f, -C1, -C2, -C3, -C4, -C5};
+  if constexpr (k == 0) return a;
+  else if constexpr (k == 12) return make_float2(-a.x, -a.y);
+  else if constexpr (k == 6) return INV ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
+  else if constexpr (k == 18) return INV ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
+  else {
+    constexpr float wr = cs[k];
+    constexpr float wi = INV ? sn[k] : -sn[k];
+    return make_float2(a.x * wr - a.y * wi, a.x * wi + a.y * wr);
+  }
+}
+
+// X0 = a + b + c,  X1 = a + b w + c w^2,  X2 = a + b w^2 + c w,  w = e^{-+ 2 pi i/3}
+template <bool INV>
+__device__ __forceinline__ void dft3(float2& a, float2& b, float2& c) {
+  constexpr float h = 0.86602540378443865f;   // sqrt(3)/2
+  const float2 s = c_add(b, c), d = c_sub(b, c);
+  const float2 m = make_float2(a.x - 0.5f * s.x, a.y - 0.5f * s.y);
+  const float2 n = INV ? make_float2(-h * d.y, h * d.x) : make_float2(h * d.y, -h * d.x);   // (+-i) h d
+  a = c_add(a, s); b = c_add(m, n); c = c_sub(m, n);
+}
+
+template <int B, int C, bool INV> struct Twiddle24 {
+  static __device__ __forceinline__ void run(float2 (&y)[3][8]) {
+    y[B][C] = mul_w24<B * C, INV>(y[B][C]);
+    if constexpr (C + 1 < 8) Twiddle24<B, C + 1, INV>::run(y);
+    else if constexpr (B + 1 < 3) Twiddle24<B + 1, 1, INV>::run(y);
+  }
+};
+
+// n = 3a + b (a < 8, b < 3), k = c + 8d (c < 8, d < 3):  W24^{nk} = W8^{ac} W24^{bc} W3^{bd};  natural order in and out
+template <bool INV>
+__device__ __forceinline__ void dft24(float2 (&v)[24]) {
+  float2 y[3][8];
+#pragma unroll
+  for (int b = 0; b < 3; ++b) {
+#pragma unroll
+    for (int a = 0; a < 8; ++a) y[b][a] = v[3 * a + b];
+    dft8<INV>(y[b]);                          // Y_b[c]
+  }
+  Twiddle24<1, 1, INV>::run(y);               // Y_b[c] *= W24^{bc}
+#pragma unroll
+  for (int c = 0; c < 8; ++c) {
+    dft3<INV>(y[0][c], y[1][c], y[2][c]);     // d = 0, 1, 2
+    v[c] = y[0][c]; v[c + 8] = y[1][c]; v[c + 16] = y[2][c];
+  }
+}
+
 template <int R, bool INV>
 __device__ __forceinline__ void dft(float2 (&v)[R]) {
-  static_assert(R == 2 || R == 4 || R == 8 || R == 16, "radix");
+  static_assert(R == 2 || R == 4 || R == 8 || R == 16 || R == 24, "radix");
   if constexpr (R == 2) dft2<INV>(v[0], v[1]);
   else if constexpr (R == 4) dft4<INV>(v[0], v[1], v[2], v[3]);
   else if constexpr (R == 8) dft8<INV>(v);
-  else dft16<INV>(v);
+  else if constexpr (R == 16) dft16<INV>(v);
+  else dft24<INV>(v);
 }
 
 // Per-thread twiddles w[q] = e^{-2 pi i j q/N}, q < E, from a table tw[k] = e^{-2 pi i k/N} (k < N).
@@ -121,6 +178,14 @@ __device__ __forceinline__ void load_twiddles(float2 (&w)[E], const float2* __re
 // stage 1: radix-E butterfly over the thread's registers, then the twiddle W_N^{jq}
 template <int E, bool INV>
 __device__ __forceinline__ void fft_stage1(float2 (&v)[E], const float2 (&w)[E]) {
+  dft<E, INV>(v);
+#pragma unroll
+  for (int q = 1; q < E; ++q) v[q] = INV ? c_mulc(v[q], w[q]) : c_mul(v[q], w[q]);
+}
+
+// the same with the twiddles read from a table (shared memory) where E registers for them are too many
+template <int E, bool INV>
+__device__ __forceinline__ void fft_stage1(float2 (&v)[E], const float2* __restrict__ w) {
   dft<E, INV>(v);
 #pragma unroll
   for (int q = 1; q < E; ++q) v[q] = INV ? c_mulc(v[q], w[q]) : c_mul(v[q], w[q]);

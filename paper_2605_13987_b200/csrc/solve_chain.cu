@@ -125,6 +125,7 @@ Plan make_plan(int nx, int ny, int nz, int L, bool force_generic) {
     if (nx == 32) set_plane<32, 8>(p);
     else if (nx == 64) set_plane<64, 8>(p);
     else if (nx == 128) set_plane<128, 16>(p);
+    else if (nx == 96) set_plane<96, 24>(p);       // configs[4]: radix-3 register transform (dft24 x dft4)
   }
   if (!p.plane_fast) {
     p.plane_step = k_plane<false>;
@@ -156,7 +157,7 @@ void chain_describe(const wt_geometry* g, std::string* out) {
   const Plan p = make_plan(g->nx, g->ny, g->nz, (int)g->layers.size(), env_flag("WTIDE_GENERIC"));
   const int B = (int)g->pad_pot.size();
   *out = std::string("chain: ") + (p.plane_fast ? "k_plane_fast" : "k_plane") + " + " + (p.line_fast ? (env_flag("WTIDE_PENCIL1") ? "k_pencil" : "k_pencil2") : "k_spectral") +
-         " + " + ((B > 640 || env_flag("WTIDE_SPLIT_BOUNDARY")) ? "k_boundary<1|2|3>" : (p.plane_fast && g->nx == g->ny ? "k_boundary_fast (cluster)" : "k_boundary_cluster")) +
+         " + " + ((B > 640 || env_flag("WTIDE_SPLIT_BOUNDARY")) ? "k_boundary<1|2|3>" : (p.plane_fast && g->nx == g->ny && g->nx != 96 ? "k_boundary_fast (cluster)" : "k_boundary_cluster")) +
          ", CUDA graph per output step";
 }
 

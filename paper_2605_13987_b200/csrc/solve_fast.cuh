@@ -33,7 +33,7 @@ template <int N> struct PlaneCfg {
 // Exchanges ping-pong between two buffers P and Q: six barriers per plane.
 // ------------------------------------------------------------------------------------------------
 template <int N, int E, bool EMIT>
-__global__ void __launch_bounds__(N * N / (2 * E), (N <= 64) ? 3 : 1)   // 80 registers, no spills (4 CTAs/SM at 64 registers spilled and measured 1 us slower per substep)
+__global__ void __launch_bounds__(N * N / (2 * E), (N <= 64) ? 3 : (N == 96 ? 2 : 1))   // 80 registers, no spills (4 CTAs/SM at 64 registers spilled and measured 1 us slower per substep)
 k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
   using C = PlaneCfg<N>;
   constexpr int Y2 = C::Y2, T = N / E, SX = C::SX, SU = C::SU, BUF = C::BUF;
@@ -49,8 +49,17 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
   float2* Q = P + BUF;
   const int L = g.L;
 
-  float2 w[E];
-  load_twiddles<E>(w, g.twx, j);          // N x N plane: twx == twy
+  // per-thread twiddles W_N^{jq}: registers for E <= 16; a [T][E] table in shared memory for E = 24 (N = 96), where 48 more
+  // registers would leave one CTA per SM
+  constexpr bool TW_SMEM = E > 16;
+  __shared__ float2 s_w[TW_SMEM ? T * E : 1];
+  float2 w_reg[TW_SMEM ? 1 : E];
+  const float2* w_tab = s_w + (TW_SMEM ? j * E : 0);
+  if constexpr (TW_SMEM) {
+    for (int i = tid; i < T * E; i += N * N / (2 * E)) s_w[i] = __ldg(g.twx + (i / E) * (i % E));   // N x N plane: twx == twy
+  } else {
+    load_twiddles<E>(w_reg, g.twx, j);
+  }
   // small tables that are needed in the middle and at the end of the kernel go to shared memory now, while the
   // predecessor is still running: a global load there would stall every warp of the CTA with nothing to overlap
   __shared__ float s_sdt[256];
@@ -102,7 +111,7 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
     }
   }
   // ---- A: inverse transform along x ---------------------------------------------------------------------
-  fft_stage1<E, true>(X, w);
+  if constexpr (TW_SMEM) fft_stage1<E, true>(X, w_tab); else fft_stage1<E, true>(X, w_reg);
 #pragma unroll
   for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[q];
   __syncthreads();
@@ -128,7 +137,7 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
     }
   }
   // ---- B: inverse transform along y -> E at the nodes (rows 2 ln | 2 ln + 1, y = j + T r) -----------------
-  fft_stage1<E, true>(X, w);
+  if constexpr (TW_SMEM) fft_stage1<E, true>(X, w_tab); else fft_stage1<E, true>(X, w_reg);
 #pragma unroll
   for (int q = 0; q < E; ++q) P[(q * T + j) * Y2 + ln] = X[q];
   __syncthreads();
@@ -148,7 +157,7 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
     X[r].y *= s_sdt[sid[r] >> 8];
   }
   // ---- C: forward transform along y ---------------------------------------------------------------------
-  fft_stage1<E, false>(X, w);
+  if constexpr (TW_SMEM) fft_stage1<E, false>(X, w_tab); else fft_stage1<E, false>(X, w_reg);
 #pragma unroll
   for (int q = 0; q < E; ++q) Q[(q * T + j) * Y2 + ln] = X[q];
   __syncthreads();
@@ -169,7 +178,7 @@ k_plane_fast(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
     }
   }
   // ---- D: forward transform along x ---------------------------------------------------------------------
-  fft_stage1<E, false>(X, w);
+  if constexpr (TW_SMEM) fft_stage1<E, false>(X, w_tab); else fft_stage1<E, false>(X, w_reg);
 #pragma unroll
   for (int q = 0; q < E; ++q) Q[(q * T + j) * Y2 + ln] = X[q];
   __syncthreads();

@@ -151,7 +151,8 @@ def test_every_config_geometry_on_a_reduced_grid():
 @pytest.mark.parametrize("which,grid,nt,env", [
     ("sweep1", (64, 64, 8), 4, {}),      # 598 pads: cluster path, the CTA's slice of Ainv does NOT fit in shared memory
     ("sweep7", (64, 64, 8), 4, {}),      # 2570 pads (pitch 25 um, bias radius 10 um): k_boundary<1|2|3>, 53 MB inverse
-    ("cfg4", (96, 96, 12), 4, {}),       # 846 pads on the radix-3 xy grid of configs[4]: size-generic kernels + k_boundary<1|2|3>
+    ("cfg4", (96, 96, 12), 4, {}),       # 846 pads on the radix-3 xy grid of configs[4]: k_plane_fast<96> (dft24 x dft4) + k_spectral + k_boundary<1|2|3>
+    ("cfg4", (96, 96, 12), 4, {"WTIDE_GENERIC": "1"}),   # the same through the size-generic plane kernel
     ("sweep3", (64, 64, 8), 4, {"WTIDE_CHAIN": "1"}),   # 1018 pads through the kernel chain
     ("sweep3", (64, 64, 8), 4, {}),      # 1018 pads
 ])
@@ -214,7 +215,7 @@ def _start_oracles_early(request):
 def test_full_grid_window_matches_the_oracle(name, full_size_oracles):
     """BASELINE.json configs[1], [2] and [4] exactly as bench.py runs them -- full grid AND full nt (6.4 GB, 51.5 GB and
     43.5 GB tables: offsets beyond 2^32 bytes and 2^31 floats), cfg 1/2 on the persistent register-FFT solver, cfg 4 on the
-    size-generic radix-3 kernels with the three-launch boundary adjust for its 846 pads -- and the first time samples of
+    radix-3 register-FFT plane kernel, the size-generic z-line kernel with the three-launch boundary adjust for its 846 pads -- and the first time samples of
     the table against the oracle over the WHOLE grid (H[n] does not depend on later steps, so the oracle only has to
     produce the window)."""
     spec = FULL_SIZE[name]
@@ -222,7 +223,7 @@ def test_full_grid_window_matches_the_oracle(name, full_size_oracles):
     nt = spec["nt"]
     g = wt.wt_make_geometry(d_full)
     plan = wt.wt_describe_plan(g)
-    assert plan.startswith("persistent" if name in ("cfg1", "cfg2") else "chain: k_plane + k_spectral + k_boundary<1|2|3>"), plan
+    assert plan.startswith("persistent" if name in ("cfg1", "cfg2") else "chain: k_plane_fast + k_spectral + k_boundary<1|2|3>"), plan
     (H,) = wt.wt_solve_H([g])
     torch.cuda.synchronize()
     h = H[:, :, :, :nt].contiguous().cpu().numpy()
