@@ -471,6 +471,26 @@ def run_ours(args):
     barrier()
     e2e_s = (time.perf_counter() - t0) / args.steps
 
+    # ---- SURVEY 8(f) row 1 beside the step (not part of it): the electrostatic field of the same geometry, readout column at
+    # 1 V and the others at 0 V, preconditioned CG to a residual of 1e-7; one cooperative launch, timed with events
+    static_info = None
+    if rank == 0 and not args.no_static:
+        pots = [1.0 if c["role"] == wt.WT_READOUT else 0.0 for c in d["columns"]]
+        best = None
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record(side)
+            _, es_lap, info = wt.wt_solve_static(g, pots, precondition=True, max_iter=4000, tol=1e-7, want_v=False, device=dev)
+            e1.record(side)
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            best = ms if best is None else min(best, ms)
+        info = info.cpu().numpy()
+        static_info = {"ms": best, "iterations": int(info[0]), "relative_residual": float(info[1]),
+                       "us_per_iteration": 1e3 * best / max(1, int(info[0])), "what": "wt_solve_static, preconditioned CG, two V <-> rho round trips per iteration"}
+        del es_lap
+
     # ---- reduce over ranks (max time, summed work)
     (solve_ms, conv_ms, step_ms, e2e_ms), total_terms = reduce_over_ranks([solve_ms, conv_ms, step_ms, e2e_s * 1e3], terms, world, dev)
 
@@ -512,6 +532,8 @@ def run_ours(args):
                            "carriers": n_car, "carrier_steps": n_steps_total,
                            "mean_steps": n_steps_total / max(1, n_car)}}
         stages["solve"]["plan"] = plan
+        if static_info:
+            stages["static_field"] = static_info
         stages["setup_s"] = setup_s
         line = {"metric": METRIC, "value": total_terms / (conv_ms * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
                 "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -749,6 +771,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference", "cufft"])
+    ap.add_argument("--no-static", action="store_true", help="skip the timing of wt_solve_static (reported under stages.static_field)")
     ap.add_argument("--tracks", type=int, default=1000, help="MIP tracks per GPU")
     ap.add_argument("--carriers", type=int, default=1000, help="macro-carriers per track")
     ap.add_argument("--config", type=int, default=1, choices=[0, 1, 2, 3, 4],

@@ -67,6 +67,14 @@ typedef struct {
   int    substeps;     /* forward-Euler substeps per dt; 0 = auto = ceil(dt*sigma_max/eps) (R12)  */
   int    n_columns;
   const wt_column* columns; /* host array, borrowed for the duration of the call only            */
+  int    mirror_z;     /* 0: the box is periodic in z (R7).  1: z = 0 and z = lz are mirror (Neumann) surfaces, by the method of
+                          images: the handle describes the DOUBLED box lz' = 2 lz, nz' = 2 nz (node spacing
+                          unchanged; nodes 0 and nz lie on the mirror planes) with the columns j < n_columns as given and
+                          their images n_columns + j at z in [2 lz - z1, 2 lz - z0].  An image carries its own contact pad (on
+                          the mirrored layer) unless the column's pad layer lies on a mirror plane (layer 0 or nz), where the
+                          pad is its own image and the image column is a WT_SEGMENT.  Every query, table size and H layout is
+                          that of the doubled box; the sensor is its first half, z in [0, lz] = layers 0 .. nz (layer nz
+                          exists: interpolation up to z = lz needs no clamp).  Needs 2 nz <= 1024, 2 n_columns <= 127. */
 } wt_geometry_desc;
 
 /* Steps a0 (setup) of SURVEY.md section 8(a): voxelise the columns (node-centre test, minimum image
@@ -188,6 +196,8 @@ int wt_conv_workspace_bytes(const wt_geometry* geom, int64_t n_tracks, int64_t n
 #define WT_Q_N_CONDUCTING          6  /* nodes with sigma > 0                                    */
 #define WT_Q_N_PAD_LAYERS          7  /* distinct z-layers holding pads                          */
 #define WT_Q_NT                    8
+#define WT_Q_N_COLUMNS             9  /* columns of the handle (2 n_columns of the descriptor with mirror_z)  */
+#define WT_Q_NZ                   10  /* z layers of the handle (2 nz of the descriptor with mirror_z)        */
 int wt_query(const wt_geometry* geom, int what, int64_t* value);
 
 /* Host copies of setup results (for checks against an independent voxeliser):

@@ -395,6 +395,33 @@ def static_potential(desc, column_potentials):
 
 
 # ----------------------------------------------------------------------------------------
+# mirror (Neumann) surfaces at z = 0 and z = lz by the method of images
+# ----------------------------------------------------------------------------------------
+def mirror_z_desc(desc):
+    """A field with dV/dz = 0 on the planes z = 0 and z = lz is the restriction to 0 <= z <= lz of a field that is even about
+    both planes, hence periodic with period 2 lz: the mirror-surface problem IS the periodic problem (R7) on the doubled box
+    lz' = 2 lz, nz' = 2 nz (same node spacing; nodes 0 and nz on the planes) holding every column and its image at
+    z in [2 lz - z1, 2 lz - z0].  Columns j < n stay as given, images are columns n + j.  The image of a contact pad is a
+    contact pad on the mirrored layer; a pad layer on a mirror plane (layer 0 or nz) is its own image, and the image column
+    then carries none (WT_SEGMENT).  Returns the descriptor of the doubled box (mirror_z cleared)."""
+    n = len(desc["columns"])
+    lz2, nz2 = 2.0 * desc["lz"], 2 * desc["nz"]
+    z = node_coordinates(nz2, lz2)
+    cols = [dict(c) for c in desc["columns"]]
+    for c in desc["columns"]:
+        inside = np.nonzero((c["z0"] <= z) & (z <= c["z1"]))[0]
+        kpad = int(inside[-1] if c["pad_at_z1"] else inside[0])
+        im = dict(c, z0=lz2 - c["z1"], z1=lz2 - c["z0"], pad_at_z1=0 if c["pad_at_z1"] else 1)
+        if c["role"] != WT_SEGMENT and kpad in (0, desc["nz"]):
+            im["role"] = WT_SEGMENT
+        cols.append(im)
+    assert len(cols) == 2 * n
+    d = dict(desc, lz=lz2, nz=nz2, columns=cols)
+    d["mirror_z"] = 0
+    return d
+
+
+# ----------------------------------------------------------------------------------------
 # SURVEY 8(f)-2: carrier transport in the solved field (PAPER.md:73 "computing the paths of the carriers",
 # :101 "dominates the time-to-insight"; BASELINE.json configs[1]: saturated-drift model
 # v = mu E / (1 + mu E / v_sat), mu_e = 1800, mu_h = 1500 cm^2/Vs, v_sat = 1.5e7 cm/s, up to nt steps)

@@ -17,7 +17,7 @@ from . import build as _build
 WT_OK, WT_EINVAL, WT_EGEOM, WT_EUNSTABLE, WT_ENOMEM, WT_ECUDA = 0, -1, -2, -3, -4, -5
 WT_BIAS, WT_READOUT, WT_SEGMENT = 0, 1, 2
 WT_Q_H_BYTES, WT_Q_SOLVE_WORKSPACE_BYTES, WT_Q_SUBSTEPS, WT_Q_N_PADS = 1, 2, 3, 4
-WT_Q_N_NODES, WT_Q_N_CONDUCTING, WT_Q_N_PAD_LAYERS, WT_Q_NT = 5, 6, 7, 8
+WT_Q_N_NODES, WT_Q_N_CONDUCTING, WT_Q_N_PAD_LAYERS, WT_Q_NT, WT_Q_N_COLUMNS, WT_Q_NZ = 5, 6, 7, 8, 9, 10
 WT_A_COLUMN_ID, WT_A_PAD_NODES, WT_A_PAD_POTENTIAL, WT_A_AINV, WT_A_GT, WT_A_GZT = 1, 2, 3, 4, 5, 6
 
 EXPORTS = ("wt_make_geometry", "wt_solve_H", "wt_convolve_currents", "wt_free", "wt_trajectory_nodes",
@@ -34,7 +34,7 @@ class wt_geometry_desc(C.Structure):
     _fields_ = [("lx", C.c_double), ("ly", C.c_double), ("lz", C.c_double),
                 ("nx", C.c_int), ("ny", C.c_int), ("nz", C.c_int), ("nt", C.c_int),
                 ("dt", C.c_double), ("eps_r", C.c_double), ("v_w", C.c_double),
-                ("substeps", C.c_int), ("n_columns", C.c_int), ("columns", C.POINTER(wt_column))]
+                ("substeps", C.c_int), ("n_columns", C.c_int), ("columns", C.POINTER(wt_column)), ("mirror_z", C.c_int)]
 
 
 class WtideError(RuntimeError):
@@ -124,10 +124,13 @@ def wt_make_geometry(desc: dict) -> Geometry:
     for i, c in enumerate(desc["columns"]):
         cols[i] = wt_column(c["cx"], c["cy"], c["radius"], c["resistivity"], c["z0"], c["z1"], c["role"], c["pad_at_z1"])
     d = wt_geometry_desc(desc["lx"], desc["ly"], desc["lz"], desc["nx"], desc["ny"], desc["nz"], desc["nt"],
-                         desc["dt"], desc["eps_r"], desc["v_w"], desc.get("substeps", 0), len(cols), cols)
+                         desc["dt"], desc["eps_r"], desc["v_w"], desc.get("substeps", 0), len(cols), cols, int(desc.get("mirror_z", 0)))
     out = C.c_void_p()
     _check(_lib.wt_make_geometry(C.byref(d), C.byref(out)))
-    return Geometry(out.value, dict(desc))
+    kept = dict(desc)
+    if kept.get("mirror_z", 0):       # the handle describes the doubled box (include/wtide.h): shapes follow it
+        kept["nz"], kept["lz"] = 2 * desc["nz"], 2.0 * desc["lz"]
+    return Geometry(out.value, kept)
 
 
 def wt_free(geom: Geometry):

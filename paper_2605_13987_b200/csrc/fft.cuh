@@ -1,4 +1,4 @@
-// Shared-memory mixed-radix (4, 2, 3) Stockham FFT building block for libwtide's spectral solve.
+// Shared-memory mixed-radix (8, 4, 2, 3) Stockham FFT building block for libwtide's spectral solve.
 //
 // PAPER.md:95 uses "the 3D FFT implementation shipped with CUDA" (cuFFT); here the 3-D transform is
 // split into z-line and xy-plane kernels that keep a tile in shared memory and fuse the per-mode
@@ -43,6 +43,24 @@ template <typename C2> struct Butterfly<4, C2> {
     C2 t0 = cadd(v[0], v[2]), t1 = csub(v[0], v[2]);
     C2 t2 = cadd(v[1], v[3]), t3 = crot(csub(v[1], v[3]), inverse);
     v[0] = cadd(t0, t2); v[1] = cadd(t1, t3); v[2] = csub(t0, t2); v[3] = csub(t1, t3);
+  }
+};
+template <typename C2> struct Butterfly<8, C2> {
+  // even / odd halves by two radix-4 butterflies, then X[k] = E[k] + W8^k O[k], X[k+4] = E[k] - W8^k O[k]
+  static __device__ __forceinline__ void run(C2* v, bool inverse) {
+    using T = typename scalar_of<C2>::type;
+    const T h = (T)0.70710678118654752440;
+    C2 e[4] = {v[0], v[2], v[4], v[6]}, o[4] = {v[1], v[3], v[5], v[7]};
+    Butterfly<4, C2>::run(e, inverse);
+    Butterfly<4, C2>::run(o, inverse);
+    const T s = inverse ? (T)1 : (T)-1;            // W8 = (1 + s i)/sqrt(2)
+    const C2 o1 = cmake<C2>(h * (o[1].x - s * o[1].y), h * (o[1].y + s * o[1].x));
+    const C2 o2 = crot(o[2], inverse);
+    const C2 o3 = cmake<C2>(h * (-o[3].x - s * o[3].y), h * (-o[3].y + s * o[3].x));   // W8^3 = (-1 + s i)/sqrt(2)
+    v[0] = cadd(e[0], o[0]); v[4] = csub(e[0], o[0]);
+    v[1] = cadd(e[1], o1);   v[5] = csub(e[1], o1);
+    v[2] = cadd(e[2], o2);   v[6] = csub(e[2], o2);
+    v[3] = cadd(e[3], o3);   v[7] = csub(e[3], o3);
   }
 };
 template <typename C2> struct Butterfly<3, C2> {
@@ -97,6 +115,10 @@ template <typename C2>
 __device__ __forceinline__ C2* fft_lines(C2* a, C2* b, int L, int n_lines, int ls, int es, const C2* __restrict__ tw,
                                          bool inverse) {
   int Ns = 1, rem = L;
+  while (rem % 8 == 0) {
+    fft_pass<8, C2>(a, b, L, Ns, n_lines, ls, es, tw, inverse);
+    C2* t = a; a = b; b = t; Ns *= 8; rem /= 8;
+  }
   while (rem % 4 == 0) {
     fft_pass<4, C2>(a, b, L, Ns, n_lines, ls, es, tw, inverse);
     C2* t = a; a = b; b = t; Ns *= 4; rem /= 4;
@@ -115,6 +137,7 @@ __device__ __forceinline__ C2* fft_lines(C2* a, C2* b, int L, int n_lines, int l
 // number of passes fft_lines() runs for length L (parity of the ping-pong)
 __host__ __device__ inline int fft_num_passes(int L) {
   int p = 0;
+  while (L % 8 == 0) { ++p; L /= 8; }
   while (L % 4 == 0) { ++p; L /= 4; }
   if (L % 2 == 0) { ++p; L /= 2; }
   while (L % 3 == 0) { ++p; L /= 3; }

@@ -201,6 +201,33 @@ extern "C" int wt_make_geometry(const wt_geometry_desc* d, wt_geometry** out) {
     wt_set_error("wt_make_geometry: need 1..127 columns"); return WT_EINVAL;
   }
   if (d->substeps < 0) { wt_set_error("wt_make_geometry: substeps < 0"); return WT_EINVAL; }
+  if (d->mirror_z) {
+    // Mirror (Neumann) surfaces at z = 0 and z = lz by the method of images: the even extension of the
+    // sensor about both planes is periodic with period 2 lz, so the periodic solver runs on the doubled box
+    if (d->mirror_z != 1 || 2 * d->nz > 1024 || 2 * d->n_columns > 127) {
+      wt_set_error("wt_make_geometry: mirror_z must be 0 or 1 and needs 2 nz <= 1024, 2 n_columns <= 127"); return WT_EINVAL;
+    }
+    wt_geometry_desc m = *d;
+    m.mirror_z = 0; m.lz = 2.0 * d->lz; m.nz = 2 * d->nz; m.n_columns = 2 * d->n_columns;
+    std::vector<wt_column> cols(d->columns, d->columns + d->n_columns);
+    for (int j = 0; j < d->n_columns; ++j) {
+      const wt_column& c = d->columns[j];
+      if (!(c.z0 >= 0 && c.z0 < c.z1 && c.z1 <= d->lz)) { wt_set_error("wt_make_geometry: bad column " + std::to_string(j)); return WT_EINVAL; }
+      int kfirst = -1, klast = -1;               // the column's layers on the doubled grid, as the voxeliser finds them
+      for (int k = 0; k < m.nz; ++k) {
+        const double z = ((double)k * m.lz) / m.nz;
+        if (c.z0 <= z && z <= c.z1) { if (kfirst < 0) kfirst = k; klast = k; }
+      }
+      const int kpad = c.pad_at_z1 ? klast : kfirst;
+      wt_column im = c;
+      im.z0 = m.lz - c.z1; im.z1 = m.lz - c.z0;
+      im.pad_at_z1 = c.pad_at_z1 ? 0 : 1;
+      if (c.role != WT_SEGMENT && (kpad == 0 || kpad == d->nz)) im.role = WT_SEGMENT;   // the pad is its own image
+      cols.push_back(im);
+    }
+    m.columns = cols.data();
+    return wt_make_geometry(&m, out);
+  }
   bool any_readout = false;
   for (int j = 0; j < d->n_columns; ++j) {
     const wt_column& c = d->columns[j];

@@ -297,6 +297,8 @@ extern "C" int wt_query(const wt_geometry* g, int what, int64_t* value) {
     case WT_Q_N_CONDUCTING: *value = g->n_conducting; break;
     case WT_Q_N_PAD_LAYERS: *value = (int64_t)g->layers.size(); break;
     case WT_Q_NT: *value = g->nt; break;
+    case WT_Q_N_COLUMNS: *value = g->n_columns; break;
+    case WT_Q_NZ: *value = g->nz; break;
     default: wt_set_error("wt_query: unknown item"); return WT_EINVAL;
   }
   return WT_OK;

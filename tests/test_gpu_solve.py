@@ -278,3 +278,19 @@ def test_every_electrode_as_readout_in_one_lock_step_batch():
     for h, d in ((ha, d_a), (hb, d_b)):
         assert wo.h_rel_l2(h, wo.solve_H_from_desc(d)) <= TOL
     assert np.abs(ha.astype(np.float64) + hb).max() <= 1e-4 * np.abs(ha).max()
+
+
+@pytest.mark.parametrize("grid,nt", [((12, 12, 6), 4), ((32, 32, 32), 4)])
+def test_mirror_z_surfaces_match_the_oracle(grid, nt):
+    """mirror (Neumann) surfaces at z = 0 and z = lz (wt_geometry_desc.mirror_z, method of images) through the
+    size-generic and the register-FFT kernels against the oracle's doubled box; the table is even (H_x, H_y) / odd (H_z) about
+    the planes and has no normal field on them."""
+    base = square_cell(55.0, 60.0, grid, nt, 0.005, 5.0, 1.0, 5.0, 1.0)
+    (g,), (h,) = _solve([dict(base, mirror_z=1)])
+    nz = grid[2]
+    assert h.shape[2] == 2 * nz
+    ref = wo.solve_H_from_desc(wo.mirror_z_desc(base))
+    assert wo.h_rel_l2(h, ref) <= TOL
+    scale = np.abs(h).max()
+    assert np.abs(h[:, :, 1:, :, :2] - h[:, :, :0:-1, :, :2]).max() <= 1e-4 * scale
+    assert np.abs(h[:, :, [0, nz], :, 2]).max() <= 1e-4 * scale

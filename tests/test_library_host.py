@@ -100,3 +100,22 @@ def test_segments_give_a_depth_dependent_profile_and_match_the_oracle_voxeliser(
     _, s_same, p_same, _, _ = wo.voxelize(same)
     _, s_base, p_base, _, _ = wo.voxelize(base)
     assert np.array_equal(s_same, s_base) and np.array_equal(p_same, p_base)
+
+
+def test_mirror_z_builds_the_doubled_box_of_the_oracle():
+    """mirror_z = 1 makes the handle of the doubled box (method of images) -- voxel set, pads and
+    queries equal those of the oracle's own mirror_z_desc, for pads on the mirror planes and for a pad away from them."""
+    base = reduced_desc(geometry_desc(1), grid=(16, 16, 12), nt=8)
+    off = dict(base, columns=[dict(base["columns"][0], z0=50.0, z1=400.0), base["columns"][1]])
+    for d in (base, off):
+        g = wt.wt_make_geometry(dict(d, mirror_z=1))
+        dm = wo.mirror_z_desc(d)
+        col_id, _, pads, vpad, _ = wo.voxelize(dm)
+        assert g.shape == (16, 16, 24) and wt.wt_query(g, wt.WT_Q_NZ) == 24 and wt.wt_query(g, wt.WT_Q_N_COLUMNS) == 4
+        np.testing.assert_array_equal(wt.wt_get_array(g, wt.WT_A_COLUMN_ID), col_id.astype(np.int8))
+        np.testing.assert_array_equal(wt.wt_get_array(g, wt.WT_A_PAD_NODES), pads.astype(np.int32))
+        np.testing.assert_array_equal(wt.wt_get_array(g, wt.WT_A_PAD_POTENTIAL), vpad)
+        assert wt.wt_query(g, wt.WT_Q_H_BYTES) == 16 * 16 * 24 * 8 * 12
+    with pytest.raises(wt.WtideError) as e:
+        wt.wt_make_geometry(dict(reduced_desc(geometry_desc(0), grid=(16, 16, 768), nt=8), mirror_z=1))
+    assert e.value.code == wt.WT_EINVAL

@@ -153,3 +153,66 @@ def test_static_potential_equals_the_stationary_state_on_the_columns():
     col_id, _, _, _, _ = wo.voxelize(d)
     v, _, _ = wo.static_potential(d, [d["v_w"], 0.0])
     assert np.abs(v[col_id == 0] - d["v_w"]).max() <= 1e-10 and np.abs(v[col_id == 1]).max() <= 1e-10
+
+
+# ---- mirror (Neumann) surfaces by the method of images ---------------------------------------------------
+def _mirror_cell(grid=(8, 8, 6), nt=3):
+    return square_cell(40.0, 30.0, grid, nt, 0.01, 6.0, 0.5, 6.0, 0.5)
+
+
+def test_even_extension_is_the_neumann_problem_cosine_transform_route():
+    """Independent route: with mirror planes at z = 0 and z = lz the potential of a charge is a cosine series in z.  DCT-I over
+    the layers 0 .. nz (scipy) with the same 1/(eps |kappa|^2), kappa_z = pi m / lz, and the highest cosine mode removed (it
+    is the Nyquist mode of the doubled box, R11) must equal the oracle's periodic potential of the evenly extended charge."""
+    import scipy.fft
+    d = wo.mirror_z_desc(_mirror_cell())
+    prob = wo.problem_from_desc(d)
+    nx, ny, nz2 = prob.shape
+    nz = nz2 // 2
+    rng = np.random.default_rng(5)
+    q_half = rng.standard_normal((nx, ny, nz + 1))
+    q = np.zeros(prob.shape)
+    q[:, :, :nz + 1] = q_half
+    q[:, :, nz + 1:] = q_half[:, :, nz - 1:0:-1]                      # node 2 nz - k mirrors node k
+    v = prob.potential_of_charge(q)
+    kx, rx = wo.wavenumbers(nx, d["lx"])
+    ky, ry = wo.wavenumbers(ny, d["ly"])
+    m = np.arange(nz + 1)
+    kz = np.pi * m / (d["lz"] / 2)
+    ret = rx[:, None, None] & ry[None, :, None] & (m < nz)[None, None, :]
+    k2 = kx[:, None, None] ** 2 + ky[None, :, None] ** 2 + kz[None, None, :] ** 2
+    g = np.zeros(k2.shape)
+    ok = ret & (k2 > 0)
+    g[ok] = 1.0 / (prob.eps * k2[ok])
+    qh = scipy.fft.dct(np.fft.fftn(q_half, axes=(0, 1)), type=1, axis=2)
+    v_cos = np.real(np.fft.ifftn(scipy.fft.idct(g * qh, type=1, axis=2), axes=(0, 1))) / prob.vol
+    assert np.abs(v[:, :, :nz + 1] - v_cos).max() <= 1e-11 * np.abs(v).max()
+    ez = -prob.grad_s(v)[2]
+    assert np.abs(ez[:, :, [0, nz]]).max() <= 1e-10 * np.abs(ez).max()     # no normal field on the mirror planes
+
+
+def test_mirrored_geometry_and_its_table_are_even_about_both_planes():
+    base = _mirror_cell()
+    d = wo.mirror_z_desc(base)
+    nz = base["nz"]
+    col_id, _, pad_nodes, pad_pot, pad_col = wo.voxelize(d)
+    occ = col_id >= 0
+    assert (occ[:, :, 1:] == occ[:, :, :0:-1]).all()                      # node 2 nz - k mirrors node k
+    # pads of the BASELINE-type columns (readout from z = 0, bias up to z = lz) sit on the mirror planes: their images carry none
+    assert set(pad_nodes[:, 2]) == {0, nz} and set(pad_col) == {0, 1}
+    assert [c["role"] for c in d["columns"]] == [wo.WT_READOUT, wo.WT_BIAS, wo.WT_SEGMENT, wo.WT_SEGMENT]
+    H = wo.solve_H_from_desc(d)
+    scale = np.abs(H).max()
+    assert np.abs(H[:, :, 1:, :, :2] - H[:, :, :0:-1, :, :2]).max() <= 1e-9 * scale      # H_x, H_y even
+    assert np.abs(H[:, :, 1:, :, 2] + H[:, :, :0:-1, :, 2]).max() <= 1e-9 * scale        # H_z odd
+    assert np.abs(H[:, :, [0, nz], :, 2]).max() <= 1e-9 * scale                          # and zero on the planes (Neumann)
+    # it is a different problem from the periodic one: the table of the plain cell differs by far more than any tolerance
+    Hp = wo.solve_H_from_desc(base)
+    assert wo.h_rel_l2(H[:, :, :nz], Hp) > 1e-2
+    # a pad away from the planes is imaged as a pad
+    off = dict(base, columns=[dict(base["columns"][0], z0=6.0, z1=20.0), base["columns"][1]])
+    dm = wo.mirror_z_desc(off)
+    assert dm["columns"][2]["role"] == wo.WT_READOUT and dm["columns"][2]["pad_at_z1"] == 1
+    _, _, pn, _, pc = wo.voxelize(dm)
+    k0, k2 = set(pn[pc == 0][:, 2]), set(pn[pc == 2][:, 2])
+    assert len(k0) == 1 and len(k2) == 1 and list(k0)[0] + list(k2)[0] == 2 * nz
