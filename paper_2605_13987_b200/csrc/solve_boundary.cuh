@@ -11,12 +11,13 @@
 //
 // k_boundary_cluster runs the three phases in ONE launch on a thread-block cluster of kBndCluster CTAs
 // per geometry (small pad sets: the chain is latency bound);
-// k_boundary<1|2|3> run one phase each on as many CTAs as there are work units (large pad sets:
+// k_boundary<1|2> + k_boundary_qh run one phase each on as many CTAs as there are work units (large pad sets:
 // Ainv is streamed by the whole chip).  Work units are strided over the CTAs of the launch.
 #pragma once
 #include <cooperative_groups.h>
 #include <cuda_pipeline.h>
 
+#include "fft.cuh"
 #include "solve_common.cuh"
 
 namespace wt {
@@ -31,7 +32,6 @@ namespace wt {
 constexpr int kBndCluster = 8;
 constexpr int kBndThreads = 512;
 constexpr int kBndChunks = 16;   // kx range split of phase 1
-constexpr int kBndKx = 16;       // kx values per work unit of phase 3
 
 struct BndSmem {                  // byte offsets into the dynamic shared memory
   size_t twx, twy, work, qs, ys, gx, total;
@@ -128,54 +128,87 @@ k_boundary(const __grid_constant__ GeomBatch gb, GridDev gd, int max_gl, int sub
   }
   // ---- phase 2: Q' = Ainv rhs ----------------------------------------------------------------------
   if (PHASE == 2) {
-    for (int row = cta * kWarps + warp; row < B; row += n_cta * kWarps) {
-      const double* __restrict__ a = g.ainv + (size_t)row * g.Bs;
-      double s = 0.0;
-      for (int jj = lane; jj < B; jj += 32) s += a[jj] * __ldcg(g.rhs + jj);
-#pragma unroll
-      for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-      if (lane == 0) g.q[row] = s;
-    }
-  }
-  // ---- phase 3: spectrum of the boundary charges per pad layer -------------------------------------
-  if (PHASE == 3) {
-    for (int i = tid; i < B; i += kBndThreads) qs[i] = __ldcg(g.q + i);
+    // rhs once into shared memory; a warp per row, 16-byte loads, four independent partial sums per lane (fixed order)
+    for (int i = tid; i < B; i += kBndThreads) qs[i] = __ldcg(g.rhs + i);
     __syncthreads();
-    const int kchunks = (nx + kBndKx - 1) / kBndKx;
-    int l_have = -1;
-    double2* u = work;                                  // [groups of the layer][y2]
-    for (int unit = cta; unit < g.L * kchunks; unit += n_cta) {
-      const int l = unit / kchunks, kx0 = (unit - l * kchunks) * kBndKx;
-      const int g0 = g.layer_goff[l], ng = g.layer_goff[l + 1] - g0;
-      if (l != l_have) {
-        __syncthreads();
-        for (int i = tid; i < ng * y2; i += kBndThreads) {
-          const int gi = i / y2, ky = i - gi * y2, grp = g0 + gi;
-          double2 s = make_double2(0.0, 0.0);
-          const int p0 = g.grp_off[grp], p1 = g.grp_off[grp + 1];
-          for (int p = p0; p < p1; ++p) {
-            const double2 w = twy[(ky * ys[p]) % ny];
-            const double q = qs[p];
-            s.x += q * w.x; s.y += q * w.y;
-          }
-          u[i] = s;
-        }
-        __syncthreads();
-        l_have = l;
+    const int n2 = B >> 1;
+    for (int row = cta * kWarps + warp; row < B; row += n_cta * kWarps) {
+      const double* __restrict__ a = g.ainv + (size_t)row * g.Bs;            // rows are 16-byte aligned (Bs even)
+      const double2* __restrict__ a2 = reinterpret_cast<const double2*>(a);
+      double s0 = 0.0, s1 = 0.0, s2 = 0.0, s3 = 0.0;
+      for (int jj = lane; jj < n2; jj += 64) {
+        const double2 v = a2[jj];
+        const bool more = jj + 32 < n2;
+        const double2 u = more ? a2[jj + 32] : make_double2(0.0, 0.0);
+        s0 = fma(v.x, qs[2 * jj], s0); s1 = fma(v.y, qs[2 * jj + 1], s1);
+        if (more) { s2 = fma(u.x, qs[2 * jj + 64], s2); s3 = fma(u.y, qs[2 * jj + 65], s3); }
       }
-      for (int i = tid; i < kBndKx * y2; i += kBndThreads) {
-        const int kx = kx0 + i / y2, ky = i % y2;
-        if (kx >= nx) continue;
-        double2 a = make_double2(0.0, 0.0);
-        for (int gi = 0; gi < ng; ++gi) {
-          const double2 p = dmul(u[gi * y2 + ky], twx[(kx * gx[g0 + gi]) % nx]);
-          a.x += p.x; a.y += p.y;
-        }
-        if (kx == nx / 2) a = make_double2(0.0, 0.0);   // removed Nyquist plane (R11)
-        g.qh[((size_t)l * nx + kx) * y2 + ky] = make_float2((float)(a.x * gd.inv_n), (float)(a.y * gd.inv_n));
-      }
+      if ((B & 1) && lane == 0) s0 = fma(a[B - 1], qs[B - 1], s0);
+      double sum = (s0 + s1) + (s2 + s3);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+      if (lane == 0) g.q[row] = sum;
     }
   }
+}
+
+// ------------------------------------------------------------------------------------------------
+// k_boundary_qh (phase 3 of the split boundary adjust): spectrum of the boundary point charges of one pad layer,
+//   qh[l][kx][ky] = (1/N) sum_{b in layer l} Q'_b e^{-i (kx x_b + ky y_b)},  ky < ny/2, 0 at kx = nx/2 (R11),
+// as ONE real 2-D transform of the layer's charge image in shared memory (two x-rows packed into a complex line, as in
+// k_plane) instead of a sum over the pads per mode: its cost does not grow with the pad count.  fp32: it feeds the fp32
+// fields (the persistent solver forms the same spectrum in fp32).  grid (L, n_geoms), block kBndThreads,
+// dynamic smem (2 (nx/2)(ny+1) + nx + ny) float2 + (2 nx + 1) ints.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kBndThreads)
+k_boundary_qh(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
+  pdl_trigger();
+  const GeomDev& g = gb.g[blockIdx.y];
+  const int l = blockIdx.x;
+  if (substep >= g.n_sub || g.B == 0 || l >= g.L) { pdl_wait(); return; }
+  const int nx = gd.nx, ny = gd.ny, y2 = gd.y2, hx = nx / 2, nyp = ny + 1;
+  const int tid = threadIdx.x, bd = blockDim.x;
+  extern __shared__ __align__(16) unsigned char smraw[];
+  float2* w1 = reinterpret_cast<float2*>(smraw);
+  float2* w2 = w1 + (size_t)hx * nyp;
+  float2* s_twx = w2 + (size_t)hx * nyp;
+  float2* s_twy = s_twx + nx;
+  for (int i = tid; i < nx; i += bd) s_twx[i] = g.twx[i];
+  for (int i = tid; i < ny; i += bd) s_twy[i] = g.twy[i];
+  for (int i = tid; i < hx * nyp; i += bd) w1[i] = make_float2(0.f, 0.f);
+  int* s_goff = reinterpret_cast<int*>(s_twy + ny);      // [ng + 1] pad offsets of the layer's groups (static tables: before the wait)
+  int* s_gx = s_goff + (g.lgoff[l + 1] - g.lgoff[l]) + 1;   // [ng]
+  for (int i = tid; i <= g.lgoff[l + 1] - g.lgoff[l]; i += bd) s_goff[i] = g.grp_off[g.lgoff[l] + i];
+  for (int i = tid; i < g.lgoff[l + 1] - g.lgoff[l]; i += bd) s_gx[i] = g.grp_x[g.lgoff[l] + i];
+  __syncthreads();
+  pdl_wait();
+  // the layer's charge image: pad (x, y) -> line x/2, real part for even x, imaginary part for odd x (each node holds one pad)
+  // (one thread per pad: its group, hence its x, by bisection of the layer's group offsets held in shared memory)
+  float* img = reinterpret_cast<float*>(w1);
+  {
+    const int g0 = g.lgoff[l], ng = g.lgoff[l + 1] - g0;
+    const int P0 = s_goff[0], P1 = s_goff[ng];
+    for (int p = P0 + tid; p < P1; p += bd) {
+      int lo = 0, hi = ng - 1;                         // largest k with s_goff[k] <= p
+      while (lo < hi) { const int mid = (lo + hi + 1) >> 1; if (s_goff[mid] <= p) lo = mid; else hi = mid - 1; }
+      const int x = s_gx[lo];
+      img[2 * ((x >> 1) * nyp + g.pad_y[p]) + (x & 1)] = (float)(__ldcg(g.q + p) * gd.inv_n);
+    }
+  }
+  __syncthreads();
+  float2* jf = fft_lines<float2>(w1, w2, ny, hx, nyp, 1, s_twy, false);
+  float2* jo = (jf == w1) ? w2 : w1;
+  for (int t = tid; t < hx * y2; t += bd) {
+    const int p = t / y2, k = t - p * y2;
+    const float2 zk = jf[p * nyp + k];
+    const float2 zm = jf[p * nyp + (k == 0 ? 0 : ny - k)];
+    jo[(2 * p) * y2 + k] = make_float2(0.5f * (zk.x + zm.x), 0.5f * (zk.y - zm.y));
+    jo[(2 * p + 1) * y2 + k] = make_float2(0.5f * (zk.y + zm.y), -0.5f * (zk.x - zm.x));
+  }
+  __syncthreads();
+  float2* jt = fft_lines<float2>(jo, jf, nx, y2, 1, y2, s_twx, false);
+  float2* __restrict__ out = g.qh + (size_t)l * nx * y2;
+  for (int t = tid; t < nx * y2; t += bd) out[t] = (t / y2 == nx / 2) ? make_float2(0.f, 0.f) : jt[t];   // removed Nyquist plane (R11)
 }
 
 

@@ -157,7 +157,7 @@ void chain_describe(const wt_geometry* g, std::string* out) {
   const Plan p = make_plan(g->nx, g->ny, g->nz, (int)g->layers.size(), env_flag("WTIDE_GENERIC"));
   const int B = (int)g->pad_pot.size();
   *out = std::string("chain: ") + (p.plane_fast ? "k_plane_fast" : "k_plane") + " + " + (p.line_fast ? (env_flag("WTIDE_PENCIL1") ? "k_pencil" : "k_pencil2") : "k_spectral") +
-         " + " + ((B > 640 || env_flag("WTIDE_SPLIT_BOUNDARY")) ? "k_boundary<1|2|3>" : (p.plane_fast && g->nx == g->ny && g->nx != 96 ? "k_boundary_fast (cluster)" : "k_boundary_cluster")) +
+         " + " + ((B > 640 || env_flag("WTIDE_SPLIT_BOUNDARY")) ? "k_boundary<1|2> + k_boundary_qh" : (p.plane_fast && g->nx == g->ny && g->nx != 96 ? "k_boundary_fast (cluster)" : "k_boundary_cluster")) +
          ", CUDA graph per output step";
 }
 
@@ -177,6 +177,7 @@ int chain_solve(std::vector<GeomHost>& gs, GridDev gd, int* dstep, cudaStream_t 
   const BndSmem bsm = bnd_smem(nx, ny, maxGL, maxB);
   const size_t kMaxSmem = 227 * 1024;
   const size_t sm_tr = (size_t)kStageSlots * 3 * std::max(nx, ny) * sizeof(float);
+  const size_t sm_qh = ((size_t)2 * (nx / 2) * (ny + 1) + nx + ny) * sizeof(float2) + ((size_t)2 * nx + 2) * sizeof(int);     // k_boundary_qh: one layer image, two buffers
   // boundary adjust: one cluster launch per substep for small pad sets (16 CTAs where the device can
   // co-schedule the non-portable size, else 8), three grid-wide launches otherwise
   using BndFastFn = void (*)(const GeomBatch, GridDev, const BndClSmem, int, int, double);
@@ -217,7 +218,7 @@ int chain_solve(std::vector<GeomHost>& gs, GridDev gd, int* dstep, cudaStream_t 
     if (!ok16) size_cluster(8);
     if (bcl.total > kMaxSmem) bnd_cluster = false;
   }
-  if (plan.plane_smem > kMaxSmem || plan.line_smem > kMaxSmem || bsm.total > kMaxSmem || sm_tr > kMaxSmem) {
+  if (plan.plane_smem > kMaxSmem || plan.line_smem > kMaxSmem || bsm.total > kMaxSmem || sm_tr > kMaxSmem || sm_qh > kMaxSmem) {
     wt_set_error("wt_solve_H: grid too large for the shared-memory tiles (nx*ny <= 128*128, nz <= 1024)"); return WT_EINVAL;
   }
 
@@ -247,11 +248,10 @@ int chain_solve(std::vector<GeomHost>& gs, GridDev gd, int* dstep, cudaStream_t 
   CK(set_smem((const void*)plan.line_delta, plan.line_smem));
   if (bnd_cluster) CK(set_smem(bnd_fn, bcl.total));
   CK(set_smem((const void*)k_boundary<1>, bsm.total));
-  CK(set_smem((const void*)k_boundary<2>, bsm.total)); CK(set_smem((const void*)k_boundary<3>, bsm.total));
+  CK(set_smem((const void*)k_boundary<2>, bsm.total)); CK(set_smem((const void*)k_boundary_qh, sm_qh));
   CK(set_smem((const void*)k_transpose<false>, sm_tr)); CK(set_smem((const void*)k_transpose<true>, sm_tr));
   const int n_tr = plan.plane_fast ? nz * ny : nz * nx;
   const size_t half = (size_t)nx * nz * y2;
-  const int bnd_units3 = std::max(1, maxL) * ((nx + kBndKx - 1) / kBndKx);
   const int bnd_rows = (maxB + kBndThreads / 32 - 1) / (kBndThreads / 32);
 
 #ifdef WTIDE_DEBUG   // timing experiments only (drops kernels from the substep loop: WRONG results); never in the shipped library
@@ -277,7 +277,7 @@ int chain_solve(std::vector<GeomHost>& gs, GridDev gd, int* dstep, cudaStream_t 
         launches += 3;
         note(launch(k_boundary<1>, dim3(std::max(1, maxG), nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
         note(launch(k_boundary<2>, dim3(std::max(1, bnd_rows), nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
-        note(launch(k_boundary<3>, dim3(bnd_units3, nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
+        note(launch(k_boundary_qh, dim3(std::max(1, maxL), nb), dim3(kBndThreads), sm_qh, st, pdl, 1, gb, gd, s));
       }
     }
   };
