@@ -378,6 +378,13 @@ __global__ void __launch_bounds__(kStThreads) k_static_cg(const __grid_constant_
         s2 += ri * ri; s1 += ri;
       });
       put_part(z, s2, s1);
+      if (pre) {               // the preconditioner's round trip starts on the new residual of this plane at once (no barrier)
+        const size_t base = (size_t)z * nx * ny;
+        plane_forward(a, s, z, [&](int x, int y) -> float {
+          const size_t i = base + (size_t)x * ny + y;
+          return a.mask[i] ? (float)__ldcg(a.r + i) : 0.f;
+        }, a.m0);
+      }
     }
     if (!grid_barrier()) return;
     reduce_parts(rr, sum_r);
@@ -385,8 +392,6 @@ __global__ void __launch_bounds__(kStThreads) k_static_cg(const __grid_constant_
     if (rr <= a.tol2 * bb || it >= a.max_iter) break;
     double rzn = rr;
     if (pre) {
-      phase_forward(1, false, 0.0, 0.0);
-      if (!grid_barrier()) return;
       phase_z(1);
       if (!grid_barrier()) return;
       phase_inverse(a.r);
