@@ -785,6 +785,131 @@ __device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigne
 }
 
 // ------------------------------------------------------------------------------------------------
+// RES only: pass B in two parts around the wait for the boundary charges.
+//   z_pass_b_early  (while the boundary CTAs work)  inverse z DFTs of V^_rho and -i kz V^_rho, which wait in kzb, into the
+//                   thread's registers X (field f at z = j + T r), and the values of the mixed-space fundamental solution
+//                   g~ / g~_z (kx, z - z_l, ky) the thread will need (static tables: no dependence on the charges)
+//   z_pass_b_late   (charges arrived)  S_l(kx, ky) = sum_{b in l} Q'_b e^{-i(kx x_b + ky y_b)} as in z_pass_b, then the boundary
+//                   source in MIXED space, X += sum_l (S_l / N) g~(kx, z - z_l, ky)  (a4: the translated fundamental solutions
+//                   of PAPER.md:97; the same sum the kernel chain forms in its plane kernel), and the store
+// The transform no longer waits for the charges: about 3 us per substep leave the exposed chain at configs[1].
+// ------------------------------------------------------------------------------------------------
+// (table values fetched before the wait: 32 more live registers across it spill at 128 registers per thread -- measured both ways)
+template <int LT> constexpr bool kPreG = false;
+
+template <int NZ, int E, int TYL, int LT>
+__device__ __forceinline__ void z_pass_b_early(const PersistArgs& a, int tile, unsigned char* gsm, float2 (&X)[E], float (&tv)[E][kPreG<LT> ? LT : 1],
+                                               int tid, int bar_id) {
+  using C = PencilCfg<NZ, E, TYL>;
+  using S = ZGroupSmem<NZ, E, TYL>;
+  constexpr int T = C::T, QS = C::QS, FIELD = C::FIELD, HT = C::THREADS, NT = 2 * HT;
+  const GeomDev& g = a.g;
+  const int y2 = a.gd.y2;
+  const int tiles = y2 / TYL;
+  const int kx = tile / tiles, ky0 = (tile % tiles) * TYL;
+  const int f = tid / HT, th = tid % HT;
+  const int line = th % TYL, j = th / TYL;
+  float2* buf = reinterpret_cast<float2*>(gsm + S::buf) + f * FIELD;
+  const float2* kzb = reinterpret_cast<const float2*>(gsm + S::kzb);
+  if constexpr (kPreG<LT>) {
+    const float* __restrict__ tab = (f == 0 ? g.gt : g.gzt) + (size_t)kx * NZ * y2 + ky0 + line;
+#pragma unroll
+    for (int l = 0; l < LT; ++l)
+#pragma unroll
+      for (int r = 0; r < E; ++r)
+        tv[r][l] = (l < g.L) ? __ldg(tab + (size_t)((j + T * r - g.layers[l]) & (NZ - 1)) * y2) : 0.f;
+  }
+  float2 w[E];
+  load_twiddles<E>(w, g.twz, j);
+#pragma unroll
+  for (int r = 0; r < E; ++r) X[r] = kzb[(f * NZ + j + T * r) * TYL + line];
+  fft_stage1<E, true>(X, w);
+#pragma unroll
+  for (int q = 0; q < E; ++q) buf[q * QS + j * TYL + line] = X[q];
+  group_sync(bar_id, NT);
+  fft_stage2<E, T, true>(X, j, [&](int q, int jj) { return buf[q * QS + jj * TYL + line]; });
+  // the transformed fields wait in the thread's own kzb slots (registers held across the wait spill at 128 per thread)
+  float2* kzw = reinterpret_cast<float2*>(gsm + S::kzb);
+#pragma unroll
+  for (int r = 0; r < E; ++r) kzw[(f * NZ + j + T * r) * TYL + line] = X[r];
+  group_sync(bar_id, NT);      // buf is rewritten by z_pass_b_late
+}
+
+template <int NZ, int E, int TYL, int LT>
+__device__ __forceinline__ void z_pass_b_late(const PersistArgs& a, int tile, unsigned char* gsm, float2 (&X)[E], const float (&tv)[E][kPreG<LT> ? LT : 1],
+                                              const float2* s_twxf, const float2* s_twyf, const int* s_px, const int* s_py,
+                                              float2* __restrict__ oV, float2* __restrict__ oE, int tid, int bar_id) {
+  using C = PencilCfg<NZ, E, TYL>;
+  using S = ZGroupSmem<NZ, E, TYL>;
+  constexpr int T = C::T, HT = C::THREADS, NT = 2 * HT;
+  const GeomDev& g = a.g;
+  const int nx = a.gd.nx, ny = a.gd.ny, y2 = a.gd.y2;
+  const int tiles = y2 / TYL;
+  const int kx = tile / tiles, ky0 = (tile % tiles) * TYL;
+  const int f = tid / HT, th = tid % HT;
+  const int line = th % TYL, j = th / TYL;
+  const int L = g.L, B = g.B;
+  float2* csf = reinterpret_cast<float2*>(gsm + S::buf);       // [B] Q'_b e^{-i kx x_b}
+  float2* plf = reinterpret_cast<float2*>(gsm + S::pls);       // [L][TYL] S_l(kx, ky0 + line)
+  for (int b = tid; b < B; b += NT) {
+    const float q = (float)__ldcg(g.q + b);
+    const float2 wx = s_twxf[(kx * s_px[b]) & (nx - 1)];
+    csf[b] = make_float2(q * wx.x, q * wx.y);
+  }
+  group_sync(bar_id, NT);
+  for (int i0 = 0; i0 < L * TYL; i0 += NT / 16) {
+    const int i = i0 + tid / 16, sub = tid & 15;
+    float2 s0 = make_float2(0.f, 0.f), s1 = make_float2(0.f, 0.f);
+    if (i < L * TYL) {
+      const int l = i / TYL, kyy = ky0 + i - l * TYL;
+      int b = a.lpoff[l] + sub;
+      const int be = a.lpoff[l + 1];
+      for (; b + 16 < be; b += 32) {
+        const float2 c0 = csf[b], w0 = s_twyf[(kyy * s_py[b]) & (ny - 1)];
+        const float2 c1 = csf[b + 16], w1 = s_twyf[(kyy * s_py[b + 16]) & (ny - 1)];
+        s0.x += c0.x * w0.x - c0.y * w0.y; s0.y += c0.x * w0.y + c0.y * w0.x;
+        s1.x += c1.x * w1.x - c1.y * w1.y; s1.y += c1.x * w1.y + c1.y * w1.x;
+      }
+      if (b < be) {
+        const float2 c0 = csf[b], w0 = s_twyf[(kyy * s_py[b]) & (ny - 1)];
+        s0.x += c0.x * w0.x - c0.y * w0.y; s0.y += c0.x * w0.y + c0.y * w0.x;
+      }
+    }
+    float2 sv = make_float2(s0.x + s1.x, s0.y + s1.y);
+#pragma unroll
+    for (int d = 8; d > 0; d >>= 1) { sv.x += __shfl_xor_sync(0xffffffffu, sv.x, d); sv.y += __shfl_xor_sync(0xffffffffu, sv.y, d); }
+    if (i < L * TYL && sub == 0) plf[i] = sv;
+  }
+  group_sync(bar_id, NT);
+  const float inv_n = (float)a.gd.inv_n;
+  const float* __restrict__ tab = (f == 0 ? g.gt : g.gzt) + (size_t)kx * NZ * y2 + ky0 + line;
+  {
+    const float2* kzr = reinterpret_cast<const float2*>(gsm + S::kzb);
+#pragma unroll
+    for (int r = 0; r < E; ++r) X[r] = kzr[(f * NZ + j + T * r) * TYL + line];
+  }
+#pragma unroll
+  for (int l = 0; l < LT; ++l) {
+    if (l < L) {
+      const float2 sl = make_float2(plf[l * TYL + line].x * inv_n, plf[l * TYL + line].y * inv_n);
+#pragma unroll
+      for (int r = 0; r < E; ++r) {
+        float t;
+        if constexpr (kPreG<LT>) t = tv[r][l];
+        else t = __ldg(tab + (size_t)((j + T * r - g.layers[l]) & (NZ - 1)) * y2);
+        X[r].x = fmaf(sl.x, t, X[r].x); X[r].y = fmaf(sl.y, t, X[r].y);
+      }
+    }
+  }
+  {
+    float2* __restrict__ out = (f == 0 ? oV : oE) + (size_t)kx * NZ * y2 + ky0 + line;
+#pragma unroll
+    for (int r = 0; r < E; ++r) out[(size_t)(j + T * r) * y2] = X[r];
+  }
+  group_sync(bar_id, NT);      // buf / kzb / pls are rewritten by the group's next phase
+}
+
+// ------------------------------------------------------------------------------------------------
 // The kernel.  grid = n_z_cta + n_b_cta CTAs of kPersistThreads threads (cooperative launch: all resident).
 // Dynamic shared memory: [tables][transient phase region][persistent region: fp64 state of the CTA's tiles (Z CTAs,
 // RES) | rhs, V_pad and the CTA's rows of Ainv (B CTAs)].
@@ -973,10 +1098,21 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
       }
       cta_signal(&ctl->cnt_part);
       PSTAMP();   // z2: contributions published
-      if (!cta_wait(&ctl->cnt_q, epi * (unsigned long long)a.n_b_cta, &ctl->abort, &s_ok)) return false;
-      PSTAMP();   // z3: charges arrived
-      for (int tile = my_tile; tile < n_tiles; tile += a.n_z_cta * ZG)
-        z_pass_b<NZ, EZ, TYL, LT, RES, DELTA>(a, tile, gsm, gg, s_kz, s_kzf, s_twzf, s_twxf, s_twyf, s_twz, s_twx, s_twy, s_px, s_py, oV, oE, zt, 1 + zgrp);
+      if constexpr (RES) {
+        // the group's one tile: the inverse transform runs while the boundary CTAs solve for the charges
+        float2 XB[EZ];
+        float tvb[EZ][kPreG<LT> ? LT : 1];
+        const bool have = my_tile < n_tiles;
+        if (have) z_pass_b_early<NZ, EZ, TYL, LT>(a, my_tile, gsm, XB, tvb, zt, 1 + zgrp);
+        if (!cta_wait(&ctl->cnt_q, epi * (unsigned long long)a.n_b_cta, &ctl->abort, &s_ok)) return false;
+        PSTAMP();   // z3: charges arrived
+        if (have) z_pass_b_late<NZ, EZ, TYL, LT>(a, my_tile, gsm, XB, tvb, s_twxf, s_twyf, s_px, s_py, oV, oE, zt, 1 + zgrp);
+      } else {
+        if (!cta_wait(&ctl->cnt_q, epi * (unsigned long long)a.n_b_cta, &ctl->abort, &s_ok)) return false;
+        PSTAMP();   // z3: charges arrived
+        for (int tile = my_tile; tile < n_tiles; tile += a.n_z_cta * ZG)
+          z_pass_b<NZ, EZ, TYL, LT, RES, DELTA>(a, tile, gsm, gg, s_kz, s_kzf, s_twzf, s_twxf, s_twyf, s_twz, s_twx, s_twy, s_px, s_py, oV, oE, zt, 1 + zgrp);
+      }
       PSTAMP();   // z4: pass B done
     } else {
       // ---- boundary adjust on the B CTAs: rows [r0, r1) --------------------------------------------
