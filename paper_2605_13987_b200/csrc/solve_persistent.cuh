@@ -461,6 +461,8 @@ template <int NZ, int E, int TYL> struct ZGroupSmem {
   static constexpr size_t pls = kzb + (size_t)2 * NZ * TYL * sizeof(float2);         // double2 [kMaxLayers][TYL]
   static constexpr size_t bytes = pls + (size_t)kMaxLayers * TYL * sizeof(double2);
   static constexpr size_t state_bytes = (size_t)NZ * TYL * sizeof(double2);          // RES: the tile's fp64 charge spectrum
+  static constexpr size_t gtab_bytes = (size_t)2 * NZ * TYL * sizeof(float);         // RES: the tile's slices of g~, g~_z at the head of buf during pass B
+  static_assert(gtab_bytes + 1100 * sizeof(float2) <= buf_bytes, "g slices + charge factors must fit in the exchange buffer");
   static constexpr int max_pads = (int)(kzb / 16);                                    // cs[B] double2 must fit over buf
 };
 
@@ -787,19 +789,15 @@ __device__ __forceinline__ void z_pass_b(const PersistArgs& a, int tile, unsigne
 // ------------------------------------------------------------------------------------------------
 // RES only: pass B in two parts around the wait for the boundary charges.
 //   z_pass_b_early  (while the boundary CTAs work)  inverse z DFTs of V^_rho and -i kz V^_rho, which wait in kzb, into the
-//                   thread's registers X (field f at z = j + T r), and the values of the mixed-space fundamental solution
-//                   g~ / g~_z (kx, z - z_l, ky) the thread will need (static tables: no dependence on the charges)
+//                   thread's own slots of kzb (field f at z = j + T r)
 //   z_pass_b_late   (charges arrived)  S_l(kx, ky) = sum_{b in l} Q'_b e^{-i(kx x_b + ky y_b)} as in z_pass_b, then the boundary
 //                   source in MIXED space, X += sum_l (S_l / N) g~(kx, z - z_l, ky)  (a4: the translated fundamental solutions
-//                   of PAPER.md:97; the same sum the kernel chain forms in its plane kernel), and the store
+//                   of PAPER.md:97; the same sum the kernel chain forms in its plane kernel; z_pass_b_early fetched the tile's
+//                   slices of g~, g~_z into shared memory meanwhile), and the store
 // The transform no longer waits for the charges: about 3 us per substep leave the exposed chain at configs[1].
 // ------------------------------------------------------------------------------------------------
-// (table values fetched before the wait: 32 more live registers across it spill at 128 registers per thread -- measured both ways)
-template <int LT> constexpr bool kPreG = false;
-
 template <int NZ, int E, int TYL, int LT>
-__device__ __forceinline__ void z_pass_b_early(const PersistArgs& a, int tile, unsigned char* gsm, float2 (&X)[E], float (&tv)[E][kPreG<LT> ? LT : 1],
-                                               int tid, int bar_id) {
+__device__ __forceinline__ void z_pass_b_early(const PersistArgs& a, int tile, unsigned char* gsm, float2 (&X)[E], int tid, int bar_id) {
   using C = PencilCfg<NZ, E, TYL>;
   using S = ZGroupSmem<NZ, E, TYL>;
   constexpr int T = C::T, QS = C::QS, FIELD = C::FIELD, HT = C::THREADS, NT = 2 * HT;
@@ -811,14 +809,6 @@ __device__ __forceinline__ void z_pass_b_early(const PersistArgs& a, int tile, u
   const int line = th % TYL, j = th / TYL;
   float2* buf = reinterpret_cast<float2*>(gsm + S::buf) + f * FIELD;
   const float2* kzb = reinterpret_cast<const float2*>(gsm + S::kzb);
-  if constexpr (kPreG<LT>) {
-    const float* __restrict__ tab = (f == 0 ? g.gt : g.gzt) + (size_t)kx * NZ * y2 + ky0 + line;
-#pragma unroll
-    for (int l = 0; l < LT; ++l)
-#pragma unroll
-      for (int r = 0; r < E; ++r)
-        tv[r][l] = (l < g.L) ? __ldg(tab + (size_t)((j + T * r - g.layers[l]) & (NZ - 1)) * y2) : 0.f;
-  }
   float2 w[E];
   load_twiddles<E>(w, g.twz, j);
 #pragma unroll
@@ -832,12 +822,18 @@ __device__ __forceinline__ void z_pass_b_early(const PersistArgs& a, int tile, u
   float2* kzw = reinterpret_cast<float2*>(gsm + S::kzb);
 #pragma unroll
   for (int r = 0; r < E; ++r) kzw[(f * NZ + j + T * r) * TYL + line] = X[r];
-  group_sync(bar_id, NT);      // buf is rewritten by z_pass_b_late
+  group_sync(bar_id, NT);      // (all reads of the exchange buffer done)
+  // the tile's slices of the mixed-space fundamental solution g~(kx, dz, ky), g~_z to the head of buf: static tables, so the
+  // loads fly while the boundary CTAs work; z_pass_b_late adds the boundary source from them
+  float* sg = reinterpret_cast<float*>(gsm + S::buf);
+  for (int i = tid; i < 2 * NZ * TYL; i += NT) {
+    const int ff = i / (NZ * TYL), rem = i - ff * (NZ * TYL), dz = rem / TYL, ln = rem - dz * TYL;
+    sg[i] = __ldg((ff == 0 ? g.gt : g.gzt) + ((size_t)kx * NZ + dz) * y2 + ky0 + ln);
+  }
 }
 
 template <int NZ, int E, int TYL, int LT>
-__device__ __forceinline__ void z_pass_b_late(const PersistArgs& a, int tile, unsigned char* gsm, float2 (&X)[E], const float (&tv)[E][kPreG<LT> ? LT : 1],
-                                              const float2* s_twxf, const float2* s_twyf, const int* s_px, const int* s_py,
+__device__ __forceinline__ void z_pass_b_late(const PersistArgs& a, int tile, unsigned char* gsm, float2 (&X)[E], const float2* s_twxf, const float2* s_twyf, const int* s_px, const int* s_py,
                                               float2* __restrict__ oV, float2* __restrict__ oE, int tid, int bar_id) {
   using C = PencilCfg<NZ, E, TYL>;
   using S = ZGroupSmem<NZ, E, TYL>;
@@ -849,7 +845,8 @@ __device__ __forceinline__ void z_pass_b_late(const PersistArgs& a, int tile, un
   const int f = tid / HT, th = tid % HT;
   const int line = th % TYL, j = th / TYL;
   const int L = g.L, B = g.B;
-  float2* csf = reinterpret_cast<float2*>(gsm + S::buf);       // [B] Q'_b e^{-i kx x_b}
+  const float* s_g = reinterpret_cast<const float*>(gsm + S::buf);                   // [2][NZ][TYL], written by z_pass_b_early
+  float2* csf = reinterpret_cast<float2*>(gsm + S::buf + S::gtab_bytes);             // [B] Q'_b e^{-i kx x_b}
   float2* plf = reinterpret_cast<float2*>(gsm + S::pls);       // [L][TYL] S_l(kx, ky0 + line)
   for (int b = tid; b < B; b += NT) {
     const float q = (float)__ldcg(g.q + b);
@@ -882,7 +879,7 @@ __device__ __forceinline__ void z_pass_b_late(const PersistArgs& a, int tile, un
   }
   group_sync(bar_id, NT);
   const float inv_n = (float)a.gd.inv_n;
-  const float* __restrict__ tab = (f == 0 ? g.gt : g.gzt) + (size_t)kx * NZ * y2 + ky0 + line;
+  const float* __restrict__ tab = s_g + (size_t)f * NZ * TYL + line;      // the tile's g~ (f = 0) or g~_z (f = 1), [dz][TYL]
   {
     const float2* kzr = reinterpret_cast<const float2*>(gsm + S::kzb);
 #pragma unroll
@@ -894,9 +891,7 @@ __device__ __forceinline__ void z_pass_b_late(const PersistArgs& a, int tile, un
       const float2 sl = make_float2(plf[l * TYL + line].x * inv_n, plf[l * TYL + line].y * inv_n);
 #pragma unroll
       for (int r = 0; r < E; ++r) {
-        float t;
-        if constexpr (kPreG<LT>) t = tv[r][l];
-        else t = __ldg(tab + (size_t)((j + T * r - g.layers[l]) & (NZ - 1)) * y2);
+        const float t = tab[((j + T * r - g.layers[l]) & (NZ - 1)) * TYL];
         X[r].x = fmaf(sl.x, t, X[r].x); X[r].y = fmaf(sl.y, t, X[r].y);
       }
     }
@@ -1101,12 +1096,11 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
       if constexpr (RES) {
         // the group's one tile: the inverse transform runs while the boundary CTAs solve for the charges
         float2 XB[EZ];
-        float tvb[EZ][kPreG<LT> ? LT : 1];
         const bool have = my_tile < n_tiles;
-        if (have) z_pass_b_early<NZ, EZ, TYL, LT>(a, my_tile, gsm, XB, tvb, zt, 1 + zgrp);
+        if (have) z_pass_b_early<NZ, EZ, TYL, LT>(a, my_tile, gsm, XB, zt, 1 + zgrp);
         if (!cta_wait(&ctl->cnt_q, epi * (unsigned long long)a.n_b_cta, &ctl->abort, &s_ok)) return false;
         PSTAMP();   // z3: charges arrived
-        if (have) z_pass_b_late<NZ, EZ, TYL, LT>(a, my_tile, gsm, XB, tvb, s_twxf, s_twyf, s_px, s_py, oV, oE, zt, 1 + zgrp);
+        if (have) z_pass_b_late<NZ, EZ, TYL, LT>(a, my_tile, gsm, XB, s_twxf, s_twyf, s_px, s_py, oV, oE, zt, 1 + zgrp);
       } else {
         if (!cta_wait(&ctl->cnt_q, epi * (unsigned long long)a.n_b_cta, &ctl->abort, &s_ok)) return false;
         PSTAMP();   // z3: charges arrived
