@@ -295,3 +295,16 @@ def test_mirror_z_surfaces_match_the_oracle(grid, nt):
     scale = np.abs(h).max()
     assert np.abs(h[:, :, 1:, :, :2] - h[:, :, :0:-1, :, :2]).max() <= 1e-4 * scale
     assert np.abs(h[:, :, [0, nz], :, 2]).max() <= 1e-4 * scale
+
+
+def test_three_pad_layers_on_the_persistent_kernel():
+    """More than two distinct pad layers select the kMaxLayers instantiation of the persistent kernel (pad-layer sums, charge
+    spectrum and the mixed-space boundary source loop over the layers): configs[1] grid, a third column whose pad sits inside
+    the bulk, first 4 time samples (30 Euler substeps) against the oracle over the whole grid."""
+    d = square_cell(55.0, 500.0, (64, 64, 256), 4, 0.005, 5.0, 1.0, 5.0, 1.0)
+    d["columns"].append(dict(cx=13.0, cy=41.0, radius=3.0, resistivity=1.0, z0=100.0, z1=400.0, role=wt.WT_BIAS, pad_at_z1=0))
+    (g,), (h,) = _solve([d])
+    assert wt.wt_describe_plan(g).startswith("persistent") and wt.wt_query(g, wt.WT_Q_N_PAD_LAYERS) == 3
+    ref = wo.solve_H_from_desc(d)
+    assert wo.h_rel_l2(h, ref) <= TOL
+    assert _slice_report(h, ref).max() <= 20 * TOL
