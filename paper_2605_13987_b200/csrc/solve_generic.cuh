@@ -13,15 +13,15 @@ namespace wt {
 //   forward z DFT of D~, J~z;  r^ -= D^ + i kz J^z  (a7, fp64 state);  V^ = r^/|kappa|^2  (a2);
 //   V~_rho at the pad layers in fp64 (a3);  inverse z DFT of V^ and -i kz V^  (a5, z part)
 // ------------------------------------------------------------------------------------------------
-template <bool APPLY_J, bool DELTA>
-__global__ void __launch_bounds__(256) k_spectral(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emit) {
-  pdl_trigger();
+// NZC, TYC: compile-time line length and lines per tile (0 = the run-time values): with them every index computation of the
+// Stockham passes and of the tile loops folds to constants (configs[4]: nz = 384, 8 lines per tile).
+template <bool APPLY_J, bool DELTA, int NZC, int TYC>
+__device__ __forceinline__ void spectral_body(const GeomBatch& gb, const GridDev& gd, int emit) {
   const GeomDev& g = gb.g[blockIdx.y];
-  if (substep >= g.n_sub) { pdl_wait(); return; }
-  const int nx = gd.nx, nz = gd.nz, y2 = gd.y2, TY = gd.ty;
+  const int nx = gd.nx, nz = NZC ? NZC : gd.nz, y2 = gd.y2, TY = TYC ? TYC : gd.ty;
   const int tiles = y2 / TY;
   const int kx = blockIdx.x / tiles, ky0 = (blockIdx.x % tiles) * TY;
-  const int tid = threadIdx.x, bd = blockDim.x;
+  const int tid = threadIdx.x, bd = TYC ? 32 * TYC : blockDim.x;
   const int nelem = nz * TY;
   const int L = g.L;
   extern __shared__ __align__(16) unsigned char smraw[];
@@ -121,6 +121,14 @@ __global__ void __launch_bounds__(256) k_spectral(const __grid_constant__ GeomBa
     const int z = t / TY, tyy = t - z * TY;
     mE[slab + (size_t)z * y2 + tyy] = eres[t];
   }
+}
+
+template <bool APPLY_J, bool DELTA>
+__global__ void __launch_bounds__(256) k_spectral(const __grid_constant__ GeomBatch gb, GridDev gd, int substep, int emit) {
+  pdl_trigger();
+  if (substep >= gb.g[blockIdx.y].n_sub) { pdl_wait(); return; }
+  if (gd.nz == 384 && gd.ty == 8) spectral_body<APPLY_J, DELTA, 384, 8>(gb, gd, emit);
+  else spectral_body<APPLY_J, DELTA, 0, 0>(gb, gd, emit);
 }
 
 // ------------------------------------------------------------------------------------------------
