@@ -201,7 +201,13 @@ __device__ __forceinline__ void block_sum2(double& x, double& y, double* red) {
 // ------------------------------------------------------------------------------------------------
 // k_static_cg: the whole Laplace solve.  grid = co-resident CTAs (cooperative launch), block 256.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kStThreads) k_static_cg(const __grid_constant__ StaticArgs a) {
+// NXY, NZC: the grids of BASELINE configs[1] / [3] (64 x 64 x 256), [2] (128 x 128 x 256) and [4] (96 x 96 x 384), 8 lines per z tile, with
+// compile-time sizes, so that the index arithmetic of the Stockham passes and of the pack / unpack loops folds to constants
+// (87 -> 72 us per iteration at configs[1]); NXY = 0: the sizes are run-time values
+template <int NXY, int NZC>
+__global__ void __launch_bounds__(kStThreads) k_static_cg(const __grid_constant__ StaticArgs a_in) {
+  StaticArgs a = a_in;
+  if constexpr (NXY != 0) { a.nx = NXY; a.ny = NXY; a.nz = NZC; a.y2 = NXY / 2; a.ty = 8; }
   extern __shared__ __align__(16) unsigned char smraw[];
   const int nx = a.nx, ny = a.ny, nz = a.nz, y2 = a.y2, hx = nx / 2, nyp = ny + 1;
   const int tid = threadIdx.x, bd = blockDim.x;
@@ -531,9 +537,15 @@ extern "C" int wt_solve_static(const wt_geometry* g, const double* column_potent
   cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
   if (!coop) return st_fail("device without cooperative launch", WT_ECUDA);
   if (smem > (size_t)max_smem) return st_fail("an xy-plane of this grid does not fit in shared memory", WT_EINVAL);
-  CKS(cudaFuncSetAttribute(k_static_cg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  const void* fn = (const void*)k_static_cg<0, 0>;
+  if (nx == ny && ty == 8) {
+    if (nx == 64 && nz == 256) fn = (const void*)k_static_cg<64, 256>;
+    else if (nx == 128 && nz == 256) fn = (const void*)k_static_cg<128, 256>;
+    else if (nx == 96 && nz == 384) fn = (const void*)k_static_cg<96, 384>;
+  }
+  CKS(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int per_sm = 0;
-  CKS(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_static_cg, kStThreads, smem));
+  CKS(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, fn, kStThreads, smem));
   if (per_sm < 1) return st_fail("kernel does not fit an SM", WT_ECUDA);
   const int n_tiles = nx * (y2 / ty);
   const int grid = std::min(n_sm * per_sm, std::max(nz, n_tiles));
@@ -563,7 +575,7 @@ extern "C" int wt_solve_static(const wt_geometry* g, const double* column_potent
   a.part = (double*)(b + lo.part); a.ctl = (StaticCtl*)(b + lo.ctl);
   a.V = V_dev; a.E = E_dev; a.info = info_dev;
   void* kargs[] = {(void*)&a};
-  CKS(cudaLaunchCooperativeKernel((const void*)k_static_cg, dim3(grid), dim3(kStThreads), kargs, smem, st));
+  CKS(cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(kStThreads), kargs, smem, st));
   k_static_finish<<<1, 1, 0, st>>>(a.ctl, info_dev);
   CKS(cudaGetLastError());
   g_wt_launches += 2;
