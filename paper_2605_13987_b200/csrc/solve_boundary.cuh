@@ -160,13 +160,15 @@ k_boundary(const __grid_constant__ GeomBatch gb, GridDev gd, int max_gl, int sub
 // fields (the persistent solver forms the same spectrum in fp32).  grid (L, n_geoms), block kBndThreads,
 // dynamic smem (2 (nx/2)(ny+1) + nx + ny) float2 + (2 nx + 1) ints.
 // ------------------------------------------------------------------------------------------------
+// NXY: compile-time plane size (nx = ny = NXY; 0 = run-time sizes): the index arithmetic of the passes folds to constants
+template <int NXY>
 __global__ void __launch_bounds__(kBndThreads)
 k_boundary_qh(const __grid_constant__ GeomBatch gb, GridDev gd, int substep) {
   pdl_trigger();
   const GeomDev& g = gb.g[blockIdx.y];
   const int l = blockIdx.x;
   if (substep >= g.n_sub || g.B == 0 || l >= g.L) { pdl_wait(); return; }
-  const int nx = gd.nx, ny = gd.ny, y2 = gd.y2, hx = nx / 2, nyp = ny + 1;
+  const int nx = NXY ? NXY : gd.nx, ny = NXY ? NXY : gd.ny, y2 = ny / 2, hx = nx / 2, nyp = ny + 1;
   const int tid = threadIdx.x, bd = blockDim.x;
   extern __shared__ __align__(16) unsigned char smraw[];
   float2* w1 = reinterpret_cast<float2*>(smraw);

@@ -248,7 +248,12 @@ int chain_solve(std::vector<GeomHost>& gs, GridDev gd, int* dstep, cudaStream_t 
   CK(set_smem((const void*)plan.line_delta, plan.line_smem));
   if (bnd_cluster) CK(set_smem(bnd_fn, bcl.total));
   CK(set_smem((const void*)k_boundary<1>, bsm.total));
-  CK(set_smem((const void*)k_boundary<2>, bsm.total)); CK(set_smem((const void*)k_boundary_qh, sm_qh));
+  using QhFn = void (*)(const GeomBatch, GridDev, int);
+  QhFn qh_fn = k_boundary_qh<0>;
+  if (nx == ny && nx == 64) qh_fn = k_boundary_qh<64>;
+  else if (nx == ny && nx == 96) qh_fn = k_boundary_qh<96>;
+  else if (nx == ny && nx == 128) qh_fn = k_boundary_qh<128>;
+  CK(set_smem((const void*)k_boundary<2>, bsm.total)); CK(set_smem((const void*)qh_fn, sm_qh));
   CK(set_smem((const void*)k_transpose<false>, sm_tr)); CK(set_smem((const void*)k_transpose<true>, sm_tr));
   const int n_tr = plan.plane_fast ? nz * ny : nz * nx;
   const size_t half = (size_t)nx * nz * y2;
@@ -277,7 +282,7 @@ int chain_solve(std::vector<GeomHost>& gs, GridDev gd, int* dstep, cudaStream_t 
         launches += 3;
         note(launch(k_boundary<1>, dim3(std::max(1, maxG), nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
         note(launch(k_boundary<2>, dim3(std::max(1, bnd_rows), nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
-        note(launch(k_boundary_qh, dim3(std::max(1, maxL), nb), dim3(kBndThreads), sm_qh, st, pdl, 1, gb, gd, s));
+        note(launch(qh_fn, dim3(std::max(1, maxL), nb), dim3(kBndThreads), sm_qh, st, pdl, 1, gb, gd, s));
       }
     }
   };
