@@ -52,14 +52,15 @@ __host__ __device__ inline BndSmem bnd_smem(int nx, int ny, int max_groups_per_l
 }
 
 // grid (n_cta, n_geoms_in_batch), block kBndThreads.
-template <int PHASE>
+// NXY: compile-time plane size (nx = ny = NXY; 0 = run-time sizes)
+template <int PHASE, int NXY = 0>
 __global__ void __launch_bounds__(kBndThreads)
 k_boundary(const __grid_constant__ GeomBatch gb, GridDev gd, int max_gl, int substep, int emit, double flag) {
   pdl_trigger();
   const GeomDev& g = gb.g[blockIdx.y];
   if (substep >= g.n_sub || g.B == 0) { pdl_wait(); return; }   // uniform over the geometry's CTAs
   pdl_wait();
-  const int nx = gd.nx, ny = gd.ny, y2 = gd.y2, tid = threadIdx.x;
+  const int nx = NXY ? NXY : gd.nx, ny = NXY ? NXY : gd.ny, y2 = ny / 2, tid = threadIdx.x;
   const int cta = blockIdx.x, n_cta = gridDim.x;
   const int B = g.B;
   extern __shared__ __align__(16) unsigned char smraw[];

@@ -253,6 +253,12 @@ int chain_solve(std::vector<GeomHost>& gs, GridDev gd, int* dstep, cudaStream_t 
   if (nx == ny && nx == 64) qh_fn = k_boundary_qh<64>;
   else if (nx == ny && nx == 96) qh_fn = k_boundary_qh<96>;
   else if (nx == ny && nx == 128) qh_fn = k_boundary_qh<128>;
+  using B1Fn = void (*)(const GeomBatch, GridDev, int, int, int, double);
+  B1Fn b1_fn = k_boundary<1>;
+  if (nx == ny && nx == 64) b1_fn = k_boundary<1, 64>;
+  else if (nx == ny && nx == 96) b1_fn = k_boundary<1, 96>;
+  else if (nx == ny && nx == 128) b1_fn = k_boundary<1, 128>;
+  CK(set_smem((const void*)b1_fn, bsm.total));
   CK(set_smem((const void*)k_boundary<2>, bsm.total)); CK(set_smem((const void*)qh_fn, sm_qh));
   CK(set_smem((const void*)k_transpose<false>, sm_tr)); CK(set_smem((const void*)k_transpose<true>, sm_tr));
   const int n_tr = plan.plane_fast ? nz * ny : nz * nx;
@@ -280,7 +286,7 @@ int chain_solve(std::vector<GeomHost>& gs, GridDev gd, int* dstep, cudaStream_t 
                          maxB, maxBs, ainv_in_smem, s, emit, flag));
       } else {
         launches += 3;
-        note(launch(k_boundary<1>, dim3(std::max(1, maxG), nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
+        note(launch(b1_fn, dim3(std::max(1, maxG), nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
         note(launch(k_boundary<2>, dim3(std::max(1, bnd_rows), nb), dim3(kBndThreads), bsm.total, st, pdl, 1, gb, gd, maxGL, s, emit, flag));
         note(launch(qh_fn, dim3(std::max(1, maxL), nb), dim3(kBndThreads), sm_qh, st, pdl, 1, gb, gd, s));
       }
