@@ -135,7 +135,9 @@ __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpre
 // (a carrier of configs[2] / [4] spends 2-4 steps per cell: those steps are pure FMA + shuffle, no row is read again); the
 // step table then holds (node, w * scale) pairs, the velocity and a cell key per step, and the three weights of a corner are
 // formed from the lane's rotated velocity by three multiplies.
-template <bool CACHE>
+// FULL: nt is a multiple of 128, so every lane of every warp owns three whole 16-byte groups of a row and the row loads need no
+// predicates (all BASELINE configs).
+template <bool CACHE, bool FULL>
 __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams sp) {
   const ConvParams& p = sp.c;
   const int nt = p.nt, F = 3 * nt;
@@ -151,7 +153,7 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
   unsigned long long* keys = reinterpret_cast<unsigned long long*>(smraw + kStepChunk * (8 * sizeof(float2) + sizeof(float4)));   // [kStepChunk]
 
   const int f0 = 384 * w + 4 * t;
-  const bool v0 = f0 < F, v1 = f0 + 128 < F, v2 = f0 + 256 < F;       // F % 4 == 0: whole 16-byte groups
+  const bool v0 = FULL || f0 < F, v1 = FULL || f0 + 128 < F, v2 = FULL || f0 + 256 < F;       // F % 4 == 0: whole 16-byte groups
   const int r = t % 3;
   const bool r0 = (r == 0), r1 = (r == 1);
 
@@ -434,7 +436,8 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
     // (fine time grids: nt >= 1024 in the BASELINE configs); WTIDE_CONV_CACHE=0/1 forces either kernel (both parity-tested)
     bool cache = g->nt >= 1024;
     if (const char* ev = std::getenv("WTIDE_CONV_CACHE")) cache = ev[0] == '1';
-    auto fn = cache ? k_conv_systolic<true> : k_conv_systolic<false>;
+    const bool full = g->nt % 128 == 0;
+    auto fn = cache ? (full ? k_conv_systolic<true, true> : k_conv_systolic<true, false>) : (full ? k_conv_systolic<false, true> : k_conv_systolic<false, false>);
     const size_t smem = (size_t)kStepChunk * 8 * sizeof(float4) + (size_t)nw * 3 * g->nt * sizeof(float);
     cudaError_t ea = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (ea != cudaSuccess) { wt_set_error(std::string("wt_convolve_currents: ") + cudaGetErrorString(ea)); return WT_ECUDA; }
