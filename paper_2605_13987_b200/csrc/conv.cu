@@ -143,11 +143,10 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
   const int nt = p.nt, F = 3 * nt;
   const int tid = threadIdx.x, w = tid >> 5, t = tid & 31, nw = blockDim.x >> 5;
   extern __shared__ __align__(16) unsigned char smraw[];
-  float4* tab = reinterpret_cast<float4*>(smraw);                                // [kStepChunk][8]  (node bits, c0, c1, c2)
   float* P = reinterpret_cast<float*>(smraw + kStepChunk * 8 * sizeof(float4));   // [nw][F]
   float* Pw = P + (size_t)w * F;
   __shared__ int64_t s_track;
-  // CACHE: the step table holds (node, w * scale) pairs, the velocity and the cell key of each step instead of 8 x (node, c_x, c_y, c_z)
+  // step table: per step eight (node, w * scale) pairs, the velocity and (CACHE) the cell key
   float2* tabc = reinterpret_cast<float2*>(smraw);                                // [kStepChunk][8]
   float4* tabv = reinterpret_cast<float4*>(smraw + kStepChunk * 8 * sizeof(float2));          // [kStepChunk]
   unsigned long long* keys = reinterpret_cast<unsigned long long*>(smraw + kStepChunk * (8 * sizeof(float2) + sizeof(float4)));   // [kStepChunk]
@@ -234,14 +233,6 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
       for (int j = 0; j < 3; ++j) { A[j][0] = A[j][3]; A[j][1] = sh[j][0]; A[j][2] = sh[j][1]; A[j][3] = sh[j][2]; }
     };
     // one (step, corner) entry e = (., c_x, c_y, c_z) applied to the lane's twelve floats of the corner's row
-    auto fma12 = [&](float (&D)[3][4], const float4 e, const float4 h0, const float4 h1, const float4 h2) {
-      const float q0 = r0 ? e.y : (r1 ? e.z : e.w);      // weight of component (t + x) % 3, x = 0, 1, 2
-      const float q1 = r0 ? e.z : (r1 ? e.w : e.y);
-      const float q2 = r0 ? e.w : (r1 ? e.y : e.z);
-      D[0][0] = fmaf(q0, h0.x, D[0][0]); D[0][1] = fmaf(q1, h0.y, D[0][1]); D[0][2] = fmaf(q2, h0.z, D[0][2]); D[0][3] = fmaf(q0, h0.w, D[0][3]);
-      D[1][0] = fmaf(q2, h1.x, D[1][0]); D[1][1] = fmaf(q0, h1.y, D[1][1]); D[1][2] = fmaf(q1, h1.z, D[1][2]); D[1][3] = fmaf(q2, h1.w, D[1][3]);
-      D[2][0] = fmaf(q1, h2.x, D[2][0]); D[2][1] = fmaf(q2, h2.y, D[2][1]); D[2][2] = fmaf(q0, h2.z, D[2][2]); D[2][3] = fmaf(q1, h2.w, D[2][3]);
-    };
     auto fma12q = [&](float (&D)[3][4], const float q0, const float q1, const float q2, const float4 h0, const float4 h1, const float4 h2) {
       D[0][0] = fmaf(q0, h0.x, D[0][0]); D[0][1] = fmaf(q1, h0.y, D[0][1]); D[0][2] = fmaf(q2, h0.z, D[0][2]); D[0][3] = fmaf(q0, h0.w, D[0][3]);
       D[1][0] = fmaf(q2, h1.x, D[1][0]); D[1][1] = fmaf(q0, h1.y, D[1][1]); D[1][2] = fmaf(q1, h1.z, D[1][2]); D[1][3] = fmaf(q2, h1.w, D[1][3]);
@@ -268,15 +259,13 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
             const int ix = cx ? nf.i1[0] : nf.i0[0], iy = cy ? nf.i1[1] : nf.i0[1], iz = cz ? nf.i1[2] : nf.i0[2];
             const unsigned node = ok ? (unsigned)((ix * p.ny + iy) * p.nz + iz) : 0u;
             const float ws = wgt * scale;            // a non-finite step contributes nothing (0, not 0 * inf)
+            tabc[tid * 8 + k] = make_float2(__uint_as_float(node), ok ? ws : 0.f);
             if constexpr (CACHE) {
-              tabc[tid * 8 + k] = make_float2(__uint_as_float(node), ok ? ws : 0.f);
               if (k == 0) key_hi = node;
               if (k == 7) keys[tid] = ((unsigned long long)key_hi << 32) | node;   // corners 0 and 7 identify the cell (a skipped step has both 0: never a real cell)
-            } else {
-              tab[tid * 8 + k] = make_float4(__uint_as_float(node), ok ? ws * vx : 0.f, ok ? ws * vy : 0.f, ok ? ws * vz : 0.f);
             }
           }
-          if constexpr (CACHE) tabv[tid] = ok ? make_float4(vx, vy, vz, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
+          tabv[tid] = ok ? make_float4(vx, vy, vz, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
         __syncthreads();
         for (int jm = 0; jm < mc; ++jm) {
@@ -304,12 +293,24 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
               fma12q(A, e2.w * q0, e2.w * q1, e2.w * q2, HC[2 * kk + 1][0], HC[2 * kk + 1][1], HC[2 * kk + 1][2]);
             }
           } else {
+            const float4 vv = tabv[jm];
+            const float q0 = r0 ? vv.x : (r1 ? vv.y : vv.z);      // velocity component (t + x) % 3, x = 0, 1, 2
+            const float q1 = r0 ? vv.y : (r1 ? vv.z : vv.x);
+            const float q2 = r0 ? vv.z : (r1 ? vv.x : vv.y);
+            const float4* tc4 = reinterpret_cast<const float4*>(tabc + jm * 8);
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-              const float4 e = tab[jm * 8 + k];
-              const float* __restrict__ src = p.H + (size_t)__float_as_uint(e.x) * F + f0;
-              const float4 h0 = v0 ? ldg4(src) : z4, h1 = v1 ? ldg4(src + 128) : z4, h2 = v2 ? ldg4(src + 256) : z4;
-              fma12(A, e, h0, h1, h2);
+            for (int kk = 0; kk < 4; ++kk) {
+              const float4 e2 = tc4[kk];             // (node, w * scale) of corners 2 kk and 2 kk + 1
+              {
+                const float* __restrict__ src = p.H + (size_t)__float_as_uint(e2.x) * F + f0;
+                const float4 h0 = v0 ? ldg4(src) : z4, h1 = v1 ? ldg4(src + 128) : z4, h2 = v2 ? ldg4(src + 256) : z4;
+                fma12q(A, e2.y * q0, e2.y * q1, e2.y * q2, h0, h1, h2);
+              }
+              {
+                const float* __restrict__ src = p.H + (size_t)__float_as_uint(e2.z) * F + f0;
+                const float4 h0 = v0 ? ldg4(src) : z4, h1 = v1 ? ldg4(src + 128) : z4, h2 = v2 ? ldg4(src + 256) : z4;
+                fma12q(A, e2.w * q0, e2.w * q1, e2.w * q2, h0, h1, h2);
+              }
             }
           }
           shift(m);
