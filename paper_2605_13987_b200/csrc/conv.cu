@@ -118,9 +118,10 @@ __global__ void __launch_bounds__(kThreads) k_conv_carrier(ConvParams p) {
 // One CTA handles `gc` consecutive carriers; with per_track the rows of carriers of one track are
 // summed in P (carrier order) and written as one partial row at the index of the segment's first carrier.
 // grid = ceil(n_carriers / gc), block = 32 * ceil(nt / 128) <= 256,
-// dynamic smem = kStepChunk * 8 * 16 + nw * 3 nt * 4 bytes.
+// dynamic smem = (steps per table: 32, cached kernel 128) * 8 * 16 + nw * 3 nt * 4 bytes.
 // ------------------------------------------------------------------------------------------------
-constexpr int kStepChunk = 32;
+constexpr int kStepChunk = 32;        // steps per step table: plain kernel (carriers of a few dozen steps)
+constexpr int kStepChunkCached = 128;  // cached kernel (nt >= 1024, hundreds of steps: fewer table builds, during which seven warps wait)
 
 struct SysParams {
   ConvParams c;
@@ -139,17 +140,18 @@ __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpre
 // predicates (all BASELINE configs).
 template <bool CACHE, bool FULL>
 __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams sp) {
+  constexpr int CH = CACHE ? kStepChunkCached : kStepChunk;
   const ConvParams& p = sp.c;
   const int nt = p.nt, F = 3 * nt;
   const int tid = threadIdx.x, w = tid >> 5, t = tid & 31, nw = blockDim.x >> 5;
   extern __shared__ __align__(16) unsigned char smraw[];
-  float* P = reinterpret_cast<float*>(smraw + kStepChunk * 8 * sizeof(float4));   // [nw][F]
+  float* P = reinterpret_cast<float*>(smraw + CH * 8 * sizeof(float4));   // [nw][F]
   float* Pw = P + (size_t)w * F;
   __shared__ int64_t s_track;
   // step table: per step eight (node, w * scale) pairs, the velocity and (CACHE) the cell key
-  float2* tabc = reinterpret_cast<float2*>(smraw);                                // [kStepChunk][8]
-  float4* tabv = reinterpret_cast<float4*>(smraw + kStepChunk * 8 * sizeof(float2));          // [kStepChunk]
-  unsigned long long* keys = reinterpret_cast<unsigned long long*>(smraw + kStepChunk * (8 * sizeof(float2) + sizeof(float4)));   // [kStepChunk]
+  float2* tabc = reinterpret_cast<float2*>(smraw);                                // [CH][8]
+  float4* tabv = reinterpret_cast<float4*>(smraw + CH * 8 * sizeof(float2));          // [CH]
+  unsigned long long* keys = reinterpret_cast<unsigned long long*>(smraw + CH * (8 * sizeof(float2) + sizeof(float4)));   // [CH]
 
   const int f0 = 384 * w + 4 * t;
   const bool v0 = FULL || f0 < F, v1 = FULL || f0 + 128 < F, v2 = FULL || f0 + 256 < F;       // F % 4 == 0: whole 16-byte groups
@@ -243,11 +245,11 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
     unsigned long long cell_key = ~0ULL;             // (per carrier: the first step always loads)
 
     {
-      for (int m0 = 0; m0 < M; m0 += kStepChunk) {
-        const int mc = min(kStepChunk, M - m0);
+      for (int m0 = 0; m0 < M; m0 += CH) {
+        const int mc = min(CH, M - m0);
         __syncthreads();
-        if (tid < mc) {
-          const int64_t s = s0 + m0 + tid;
+        for (int js = tid; js < mc; js += blockDim.x) {
+          const int64_t s = s0 + m0 + js;
           const float vx = p.vel[3 * s], vy = p.vel[3 * s + 1], vz = p.vel[3 * s + 2];
           const NodeFrac nf = locate(p.pos[3 * s], p.pos[3 * s + 1], p.pos[3 * s + 2], p.nx, p.ny, p.nz, p.invx, p.invy, p.invz);
           const bool ok = nf.ok && isfinite(vx) && isfinite(vy) && isfinite(vz);
@@ -259,13 +261,13 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
             const int ix = cx ? nf.i1[0] : nf.i0[0], iy = cy ? nf.i1[1] : nf.i0[1], iz = cz ? nf.i1[2] : nf.i0[2];
             const unsigned node = ok ? (unsigned)((ix * p.ny + iy) * p.nz + iz) : 0u;
             const float ws = wgt * scale;            // a non-finite step contributes nothing (0, not 0 * inf)
-            tabc[tid * 8 + k] = make_float2(__uint_as_float(node), ok ? ws : 0.f);
+            tabc[js * 8 + k] = make_float2(__uint_as_float(node), ok ? ws : 0.f);
             if constexpr (CACHE) {
               if (k == 0) key_hi = node;
-              if (k == 7) keys[tid] = ((unsigned long long)key_hi << 32) | node;   // corners 0 and 7 identify the cell (a skipped step has both 0: never a real cell)
+              if (k == 7) keys[js] = ((unsigned long long)key_hi << 32) | node;   // corners 0 and 7 identify the cell (a skipped step has both 0: never a real cell)
             }
           }
-          tabv[tid] = ok ? make_float4(vx, vy, vz, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
+          tabv[js] = ok ? make_float4(vx, vy, vz, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
         __syncthreads();
         for (int jm = 0; jm < mc; ++jm) {
@@ -439,7 +441,7 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
     if (const char* ev = std::getenv("WTIDE_CONV_CACHE")) cache = ev[0] == '1';
     const bool full = g->nt % 128 == 0;
     auto fn = cache ? (full ? k_conv_systolic<true, true> : k_conv_systolic<true, false>) : (full ? k_conv_systolic<false, true> : k_conv_systolic<false, false>);
-    const size_t smem = (size_t)kStepChunk * 8 * sizeof(float4) + (size_t)nw * 3 * g->nt * sizeof(float);
+    const size_t smem = (size_t)(cache ? kStepChunkCached : kStepChunk) * 8 * sizeof(float4) + (size_t)nw * 3 * g->nt * sizeof(float);
     cudaError_t ea = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (ea != cudaSuccess) { wt_set_error(std::string("wt_convolve_currents: ") + cudaGetErrorString(ea)); return WT_ECUDA; }
     ++g_wt_launches;
