@@ -146,7 +146,7 @@ Plan make_plan(int nx, int ny, int nz, int L, bool force_generic) {
     p.line_delta = k_spectral<false, true>;
     p.line_grid = dim3(nx * (y2 / p.ty));
     p.line_block = dim3(32 * p.ty);
-    p.line_smem = (size_t)3 * nz * p.ty * sizeof(float2) + (size_t)std::max(1, L) * p.ty * 32 * sizeof(double2) + (size_t)nz * sizeof(float2);
+    p.line_smem = (size_t)3 * nz * p.ty * sizeof(float2) + (size_t)std::max(1, L) * p.ty * 32 * sizeof(double2) + (size_t)nz * (sizeof(float2) + sizeof(double2) + sizeof(double));
   }
   return p;
 }

@@ -32,7 +32,9 @@ __device__ __forceinline__ void spectral_body(const GeomBatch& gb, const GridDev
   // twiddles of the z transform: to shared memory while the predecessor runs (every butterfly of every pass
   // would otherwise fetch them from global memory in the middle of the kernel)
   float2* s_twz = reinterpret_cast<float2*>(red + (size_t)(L > 0 ? L : 1) * TY * 32);   // [nz]
-  for (int i = tid; i < nz; i += bd) s_twz[i] = g.twz[i];
+  double2* s_twzd = reinterpret_cast<double2*>(s_twz + nz);                               // [nz] fp64 twiddles of the pad-layer sums
+  double* s_kzd = reinterpret_cast<double*>(s_twzd + nz);                                 // [nz] z wavenumbers
+  for (int i = tid; i < nz; i += bd) { s_twz[i] = g.twz[i]; s_twzd[i] = g.twzd[i]; s_kzd[i] = g.kzd[i]; }
   __syncthreads();
   pdl_wait();
   float2* mV = emit ? g.e0 : g.v0;
@@ -68,7 +70,7 @@ __device__ __forceinline__ void spectral_body(const GeomBatch& gb, const GridDev
     const int kz = t / TY;
     const size_t gi = ((size_t)kx * nz + kz) * y2 + ky;
     const bool ret = ret_x && (kz != nz / 2);
-    const double kzd = g.kzd[kz];
+    const double kzd = s_kzd[kz];
     double2 r = g.rhat[gi];
     if (APPLY_J) {
       const float2 D = dres[t], J = jres[t];
@@ -92,7 +94,7 @@ __device__ __forceinline__ void spectral_body(const GeomBatch& gb, const GridDev
 #pragma unroll
     for (int l = 0; l < kMaxLayers; ++l) {
       if (l < L) {
-        double2 w = g.twzd[(kz * g.layers[l]) % nz];
+        double2 w = s_twzd[(kz * g.layers[l]) % nz];
         w.y = -w.y;                                                    // e^{+i kz z_l}
         const double2 p = dmul(v, w);
         acc[l].x += p.x; acc[l].y += p.y;
