@@ -63,6 +63,7 @@ struct Smem {
   float2 *w1, *w2, *w3;        // plane: two buffers of hx*(ny+1); z tile: three of nz*ty (overlaid)
   float2 *twx, *twy, *twz;
   double* red;                 // [2 * kStThreads/32 + 2]
+  double* kz;                  // [nz] z wavenumbers (z tiles read one per mode)
   int* flag;
 };
 
@@ -146,7 +147,7 @@ __device__ __forceinline__ void z_tile(const StaticArgs& a, const Smem& s, int t
   const bool ret_x = (kx != nx / 2);
   for (int t = tid; t < nelem; t += bd) {
     const int kz = t / TY, ty = t - kz * TY;
-    const double kyd = a.ky[ky0 + ty], kzd = a.kz[kz];
+    const double kyd = a.ky[ky0 + ty], kzd = s.kz[kz];
     const bool ret = ret_x && (kz != nz / 2);
     const double k2 = kxd * kxd + kyd * kyd + kzd * kzd;
     double m;
@@ -223,10 +224,12 @@ __global__ void __launch_bounds__(kStThreads) k_static_cg(const __grid_constant_
     s.w2 = base + plane_buf; s.w3 = nullptr;
     s.twx = base + work; s.twy = s.twx + nx; s.twz = s.twy + ny;
     s.red = reinterpret_cast<double*>(s.twz + nz);
-    s.flag = reinterpret_cast<int*>(s.red + 2 * (kStThreads / 32) + 2);
+    s.kz = s.red + 2 * (kStThreads / 32) + 2;
+    s.flag = reinterpret_cast<int*>(s.kz + nz);
   }
   Smem sz = s;                                       // z-phase view of the same memory
   sz.w2 = s.w1 + (size_t)nz * a.ty; sz.w3 = sz.w2 + (size_t)nz * a.ty;
+  for (int i = tid; i < nz; i += bd) s.kz[i] = a.kz[i];
   for (int i = tid; i < nx + ny + nz; i += bd) {     // twiddles e^{-2 pi i k/n}
     const int n = (i < nx) ? nx : (i < nx + ny ? ny : nz);
     const int k = (i < nx) ? i : (i < nx + ny ? i - nx : i - nx - ny);
@@ -495,7 +498,7 @@ int pick_ty(int y2, int nz) {
 
 size_t st_smem(const wt_geometry* g, int ty) {
   const size_t plane = (size_t)2 * (g->nx / 2) * (g->ny + 1), zt = (size_t)3 * g->nz * ty;
-  return (std::max(plane, zt) + g->nx + g->ny + g->nz) * 8 + (2 * (kStThreads / 32) + 2) * 8 + 16;
+  return (std::max(plane, zt) + g->nx + g->ny + g->nz) * 8 + (2 * (kStThreads / 32) + 2) * 8 + (size_t)g->nz * 8 + 16;
 }
 
 int st_fail(const std::string& msg, int code) { wt_set_error("wt_solve_static: " + msg); return code; }
