@@ -917,7 +917,7 @@ template <int N, int EP, int NZ, int EZ, int TYL> struct PersistCfg {
   static constexpr bool MERGED = (N <= 64);                        // plane units carry the x and y components together
   static constexpr size_t p_bytes = (size_t)PG * (MERGED ? 3 : 2) * PlaneCfg<N>::BUF * sizeof(float2);
   static constexpr size_t z_bytes = (size_t)ZG * ZGroupSmem<NZ, EZ, TYL>::bytes;
-  static constexpr size_t t_bytes = (size_t)kStageSlots * 3 * N * sizeof(float);
+  static constexpr size_t t_bytes = (size_t)4 * kStageSlots * 3 * N * sizeof(float);   // transpose phase: four (z, y) units in flight
   static constexpr size_t phase_bytes = (p_bytes > z_bytes ? p_bytes : z_bytes) > t_bytes ? (p_bytes > z_bytes ? p_bytes : z_bytes) : t_bytes;
   static constexpr size_t state_bytes = (size_t)ZG * ZGroupSmem<NZ, EZ, TYL>::state_bytes;
 };
@@ -1154,19 +1154,31 @@ __global__ void __launch_bounds__(kPersistThreads, 1) k_persistent(const __grid_
     const int cnt = n % kStageSlots + 1, t0 = n - cnt + 1, rows = cnt * 3;
     float* tile = reinterpret_cast<float*>(phase);
     const int nt = a.gd.nt;
-    for (int unit = cta; unit < nz * ny; unit += n_cta) {
-      const int z = unit / ny, y = unit - z * ny;
-      for (int t = tid; t < rows * nx; t += kPersistThreads) {
-        const int j = t / nx, x = t - j * nx;
-        tile[t] = __ldcg(g.stage + (((size_t)j * nz + z) * ny + y) * nx + x);
+    auto run = [&](auto rows_c, auto u_c) {
+      // U (z, y) units per round, `rows` a compile-time constant where it is the full staging group (index arithmetic by constants)
+      constexpr int U = decltype(u_c)::value;
+      const int rows_ = decltype(rows_c)::value ? decltype(rows_c)::value : rows;
+      const int per = rows_ * nx;
+      for (int unit0 = cta * U; unit0 < nz * ny; unit0 += n_cta * U) {
+        const int nu = min(U, nz * ny - unit0);
+        for (int t = tid; t < nu * per; t += kPersistThreads) {
+          const int u = t / per, r = t - u * per;
+          const int unit = unit0 + u, z = unit / ny, y = unit - z * ny;
+          const int j = r / nx, x = r - j * nx;
+          tile[t] = __ldcg(g.stage + (((size_t)j * nz + z) * ny + y) * nx + x);
+        }
+        __syncthreads();
+        for (int t = tid; t < nu * per; t += kPersistThreads) {
+          const int u = t / per, r = t - u * per;
+          const int unit = unit0 + u, z = unit / ny, y = unit - z * ny;
+          const int x = r / rows_, j = r - x * rows_;
+          g.H[((((size_t)x * ny + y) * nz + z) * nt + t0) * 3 + j] = tile[u * per + j * nx + x];
+        }
+        __syncthreads();
       }
-      __syncthreads();
-      for (int t = tid; t < rows * nx; t += kPersistThreads) {
-        const int x = t / rows, j = t - x * rows;
-        g.H[((((size_t)x * ny + y) * nz + z) * nt + t0) * 3 + j] = tile[j * nx + x];
-      }
-      __syncthreads();
-    }
+    };
+    if (rows == 3 * kStageSlots) run(std::integral_constant<int, 3 * kStageSlots>{}, std::integral_constant<int, 4>{});
+    else run(std::integral_constant<int, 0>{}, std::integral_constant<int, 1>{});
   };
   // RES: the state goes back to global memory for the next launch
   auto save_state = [&]() {
