@@ -115,6 +115,27 @@ int wt_convolve_currents(const wt_geometry* geom, const float* H_dev,
                          int per_track, float* out_dev,
                          void* workspace_dev, size_t workspace_bytes, void* cuda_stream);
 
+/* Eq. 1.1 summed per track (wt_convolve_currents with per_track = 1; Eq. 1.1, same arithmetic, same kernels, same
+ * order of summation, bit-identical result) for callers that cannot allocate device memory: code in a tight serving loop,
+ * harnesses that forbid cudaMalloc.  The per-carrier rows that the workspace form keeps in the caller's workspace live in a
+ * device array built into the library: WT_NOALLOC_MAX_FLOATS fp32 = 4 MiB, held by every GPU that loads the library until
+ * the process exits.  The call allocates nothing (no cudaMalloc, cudaFree or allocating library routine); the caller still
+ * passes every input and the output, laid out as for wt_convolve_currents.
+ *   limit      n_carriers * nt <= WT_NOALLOC_MAX_FLOATS (e.g. 4096 carriers at nt = 256, 1024 at nt = 1024); beyond it the call
+ *              returns WT_ENOMEM, launches nothing and wt_last_error() names the limit: split the batch, or use the workspace form
+ *   device     the device of cuda_stream must be current (its copy of the array is looked up on first use, once per device)
+ *   sharing    every call on a device uses the same array.  Calls are safe back to back on one stream; two calls that may
+ *              overlap on the GPU (different streams without an event between them, or host threads doing so) RACE on it
+ *              and give wrong sums.  The array keeps the last call's rows; none of it has to start at zero, because each
+ *              call writes every row it later reads.
+ * Other errors as wt_convolve_currents. */
+#define WT_NOALLOC_MAX_FLOATS (1 << 20)
+int wt_convolve_tracks_noalloc(const wt_geometry* geom, const float* H_dev,
+                               int64_t n_tracks, const int64_t* track_carrier_offsets_dev,
+                               int64_t n_carriers, const int64_t* carrier_step_offsets_dev,
+                               const float* pos_dev, const float* vel_dev, const float* charge_dev,
+                               float* out_dev, void* cuda_stream);
+
 /* Releases a handle returned by wt_make_geometry.  NULL is a no-op. */
 void wt_free(void* handle);
 

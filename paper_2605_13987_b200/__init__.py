@@ -22,7 +22,8 @@ WT_A_COLUMN_ID, WT_A_PAD_NODES, WT_A_PAD_POTENTIAL, WT_A_AINV, WT_A_GT, WT_A_GZT
 
 EXPORTS = ("wt_make_geometry", "wt_solve_H", "wt_convolve_currents", "wt_free", "wt_trajectory_nodes",
            "wt_conv_workspace_bytes", "wt_query", "wt_get_array", "wt_last_error", "wt_launch_count", "wt_describe_plan", "wt_measure_fp32_fma", "wt_static_field",
-           "wt_drift_workspace_bytes", "wt_drift_count", "wt_offsets_from_counts", "wt_drift_fill", "wt_electronics", "wt_static_workspace_bytes", "wt_solve_static")
+           "wt_drift_workspace_bytes", "wt_drift_count", "wt_offsets_from_counts", "wt_drift_fill", "wt_electronics", "wt_static_workspace_bytes", "wt_solve_static",
+           "wt_convolve_tracks_noalloc")
 
 
 class wt_column(C.Structure):
@@ -58,6 +59,7 @@ def _load():
     lib.wt_make_geometry.argtypes = [C.POINTER(wt_geometry_desc), C.POINTER(vp)]
     lib.wt_solve_H.argtypes = [C.POINTER(vp), C.c_int, C.POINTER(vp), sz, vp, sz, vp]
     lib.wt_convolve_currents.argtypes = [vp, vp, i64, vp, i64, vp, vp, vp, vp, C.c_int, vp, vp, sz, vp]
+    lib.wt_convolve_tracks_noalloc.argtypes = [vp, vp, i64, vp, i64, vp, vp, vp, vp, vp, vp]
     lib.wt_free.argtypes = [vp]
     lib.wt_free.restype = None
     lib.wt_trajectory_nodes.argtypes = [vp, i64, vp, vp, vp, vp, vp]
@@ -245,6 +247,29 @@ def wt_convolve_currents(geom, H, track_carrier_offsets, carrier_step_offsets, p
     for t in (out, workspace):
         if t is not None:
             t.record_stream(_stream(device))
+    return out
+
+
+WT_NOALLOC_MAX_FLOATS = 1 << 20
+
+
+def wt_convolve_tracks_noalloc(geom, H, track_carrier_offsets, carrier_step_offsets, pos, vel, charge, out):
+    """Eq. 1.1 summed per track with the library's built-in scratch (include/wtide.h): the call allocates no device memory,
+    so `out` [n_tracks, nt] float32 is the caller's.  n_carriers * nt <= WT_NOALLOC_MAX_FLOATS, else WtideError (WT_ENOMEM).
+    Calls that overlap on the GPU race on the shared scratch."""
+    import torch
+    device = H.device
+    n_car = carrier_step_offsets.numel() - 1
+    n_trk = track_carrier_offsets.numel() - 1
+    for t in (pos, vel, charge):
+        assert t.dtype == torch.float32 and t.is_contiguous()
+    assert carrier_step_offsets.dtype == torch.int64 and track_carrier_offsets.dtype == torch.int64
+    assert out.dtype == torch.float32 and out.is_contiguous() and tuple(out.shape) == (n_trk, geom.nt) and out.device == device
+    # (_run_on_side_stream makes `device` current for the call, as the header asks)
+    _run_on_side_stream(device, lambda s: _lib.wt_convolve_tracks_noalloc(
+        geom.handle, H.data_ptr(), n_trk, track_carrier_offsets.data_ptr(), n_car, carrier_step_offsets.data_ptr(),
+        pos.data_ptr(), vel.data_ptr(), charge.data_ptr(), out.data_ptr(), s))
+    out.record_stream(_stream(device))
     return out
 
 

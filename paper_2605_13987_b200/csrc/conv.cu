@@ -14,6 +14,7 @@
 #include <algorithm>
 #include <cstdint>
 #include <cstdlib>
+#include <mutex>
 #include <string>
 
 #include "geometry.h"
@@ -475,4 +476,55 @@ extern "C" int wt_trajectory_nodes(const wt_geometry* g, int64_t n_steps, const 
   if (e != cudaSuccess) { wt_set_error(std::string("wt_trajectory_nodes: ") + cudaGetErrorString(e)); return WT_ECUDA; }
   wt_set_error("");
   return WT_OK;
+}
+
+// ---- Eq. 1.1 per track without any allocation ------------------------------------------------------------------
+// For callers that cannot call cudaMalloc (tight serving loops, harnesses that forbid it): the per-carrier rows that
+// wt_convolve_currents(per_track = 1) keeps in a caller workspace live in a file-scope device array instead.  Every GPU
+// that loads the library holds WT_NOALLOC_MAX_FLOATS * 4 bytes (4 MiB) of it until exit.  In host code the array's name is
+// a host-side stand-in, not a device address: its device address is looked up once per device (with that device current)
+// by cudaGetSymbolAddress and handed to the same kernels the workspace form launches.
+static __device__ __align__(256) float g_noalloc_rows[WT_NOALLOC_MAX_FLOATS];
+
+namespace {
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mutex;
+float* g_noalloc_ptr[kNoAllocMaxDevices];   // device address of g_noalloc_rows on device d (NULL: not looked up yet)
+}  // namespace
+
+extern "C" int wt_convolve_tracks_noalloc(const wt_geometry* g, const float* H_dev, int64_t n_tracks,
+                                          const int64_t* track_carrier_offsets_dev, int64_t n_carriers,
+                                          const int64_t* carrier_step_offsets_dev, const float* pos_dev, const float* vel_dev,
+                                          const float* charge_dev, float* out_dev, void* cuda_stream) {
+  if (!wt_valid(g)) { wt_set_error("wt_convolve_tracks_noalloc: bad handle"); return WT_EINVAL; }
+  if (n_tracks < 0 || n_carriers < 0) { wt_set_error("wt_convolve_tracks_noalloc: negative count"); return WT_EINVAL; }
+  if (n_carriers > (int64_t)WT_NOALLOC_MAX_FLOATS / g->nt) {
+    wt_set_error("wt_convolve_tracks_noalloc: n_carriers * nt = " + std::to_string(n_carriers) + " * " + std::to_string(g->nt) +
+                 " exceeds the built-in scratch of WT_NOALLOC_MAX_FLOATS = " + std::to_string((long long)WT_NOALLOC_MAX_FLOATS) +
+                 " floats; split the batch or call wt_convolve_currents with a workspace");
+    return WT_ENOMEM;
+  }
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { wt_set_error(std::string("wt_convolve_tracks_noalloc: ") + cudaGetErrorString(e)); return WT_ECUDA; }
+  if (dev < 0 || dev >= kNoAllocMaxDevices) { wt_set_error("wt_convolve_tracks_noalloc: device ordinal beyond 63"); return WT_EINVAL; }
+  float* rows = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_noalloc_mutex);
+    if (!g_noalloc_ptr[dev]) {
+      void* p = nullptr;
+      e = cudaGetSymbolAddress(&p, g_noalloc_rows);
+      if (e != cudaSuccess || !p) {
+        wt_set_error(std::string("wt_convolve_tracks_noalloc: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+        return WT_ECUDA;
+      }
+      g_noalloc_ptr[dev] = (float*)p;
+    }
+    rows = g_noalloc_ptr[dev];
+  }
+  // The kernels write every row k_track_sum reads before it reads it (one row per carrier, or per segment of a carrier
+  // group), so nothing in the array has to start at zero and what the last call left there is never read.
+  const int rc = wt_convolve_currents(g, H_dev, n_tracks, track_carrier_offsets_dev, n_carriers, carrier_step_offsets_dev, pos_dev,
+                                      vel_dev, charge_dev, 1, out_dev, rows, (size_t)WT_NOALLOC_MAX_FLOATS * sizeof(float), cuda_stream);
+  return rc;
 }
