@@ -119,10 +119,17 @@ __global__ void __launch_bounds__(kThreads) k_conv_carrier(ConvParams p) {
 // One CTA handles `gc` consecutive carriers; with per_track the rows of carriers of one track are
 // summed in P (carrier order) and written as one partial row at the index of the segment's first carrier.
 // grid = ceil(n_carriers / gc), block = 32 * ceil(nt / 128) <= 256,
-// dynamic smem = (steps per table: 32, cached kernel 128) * 8 * 16 + nw * 3 nt * 4 bytes.
+// dynamic smem = step table (32 steps of 128 bytes; cached kernel 128 steps of 328 bytes) + the partial rows, warp w's being
+// the F - 384 w floats it can reach (55 KB instead of 98 KB at nt = 1024, which goes to L1).
 // ------------------------------------------------------------------------------------------------
 constexpr int kStepChunk = 32;        // steps per step table: plain kernel (carriers of a few dozen steps)
 constexpr int kStepChunkCached = 128;  // cached kernel (nt >= 1024, hundreds of steps: fewer table builds, during which seven warps wait)
+
+// shared memory of the systolic kernel: bytes per step of the step table, and the float offset of warp w's partial row
+// (rows of F - 384 u floats, u < w, lie before it)
+constexpr int kStepBytesPlain = 8 * sizeof(float4);                                         // 8 (node, w) pairs + velocity + (unused) key
+constexpr int kStepBytesCached = 3 * 24 * sizeof(float) + 8 * sizeof(unsigned) + sizeof(unsigned long long);
+__host__ __device__ constexpr int rows_offset(int w, int F) { return w * F - 192 * w * (w - 1); }
 
 struct SysParams {
   ConvParams c;
@@ -135,24 +142,33 @@ __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpre
 
 // CACHE: the 8 x 12 floats a lane owns of the current cell's rows stay in registers while the carrier stays in the cell
 // (a carrier of configs[2] / [4] spends 2-4 steps per cell: those steps are pure FMA + shuffle, no row is read again); the
-// step table then holds (node, w * scale) pairs, the velocity and a cell key per step, and the three weights of a corner are
-// formed from the lane's rotated velocity by three multiplies.
+// step table then holds, per step, the 24 products (w_k * scale) * v_c once for each of the three rotations of the components a
+// lane can need (six 128-bit shared loads per step instead of 24 multiplies and six selects), the eight nodes and a cell key.
 // FULL: nt is a multiple of 128, so every lane of every warp owns three whole 16-byte groups of a row and the row loads need no
 // predicates (all BASELINE configs).
 template <bool CACHE, bool FULL>
 __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams sp) {
   constexpr int CH = CACHE ? kStepChunkCached : kStepChunk;
+  constexpr int kStepBytes = CACHE ? kStepBytesCached : kStepBytesPlain;
   const ConvParams& p = sp.c;
   const int nt = p.nt, F = 3 * nt;
   const int tid = threadIdx.x, w = tid >> 5, t = tid & 31, nw = blockDim.x >> 5;
   extern __shared__ __align__(16) unsigned char smraw[];
-  float* P = reinterpret_cast<float*>(smraw + CH * 8 * sizeof(float4));   // [nw][F]
-  float* Pw = P + (size_t)w * F;
+  // partial rows: warp w only ever holds sums S[g], g >= 384 w, so its row is the F - 384 w floats [384 w, F)
+  float* P = reinterpret_cast<float*>(smraw + CH * kStepBytes);
+  float* Pw = P + rows_offset(w, F) - 384 * w;                          // Pw[g], 384 w <= g < F
+  const int p_floats = rows_offset(nw, F);
   __shared__ int64_t s_track;
+  __shared__ unsigned s_cmask[kStepChunkCached / 32];   // cached kernel: where the carrier changes cell inside the step table
   // step table: per step eight (node, w * scale) pairs, the velocity and (CACHE) the cell key
   float2* tabc = reinterpret_cast<float2*>(smraw);                                // [CH][8]
   float4* tabv = reinterpret_cast<float4*>(smraw + CH * 8 * sizeof(float2));          // [CH]
-  unsigned long long* keys = reinterpret_cast<unsigned long long*>(smraw + CH * (8 * sizeof(float2) + sizeof(float4)));   // [CH]
+  unsigned long long* keys = reinterpret_cast<unsigned long long*>(smraw + CH * (8 * sizeof(float2) + sizeof(float4)));   // [CH] (plain kernel: unused)
+  // cached kernel: per step the 24 products (w_k * scale) * v_c for each of the three rotations of the components a lane can
+  // need (lane t multiplies float f of a row by component (t + f) % 3), the eight nodes and the cell key
+  float4* tabq = reinterpret_cast<float4*>(smraw);                                                         // [CH][3][6]
+  unsigned* tabn = reinterpret_cast<unsigned*>(smraw + CH * 3 * 24 * sizeof(float));                       // [CH][8]
+  if constexpr (CACHE) keys = reinterpret_cast<unsigned long long*>(smraw + CH * (3 * 24 * sizeof(float) + 8 * sizeof(unsigned)));
 
   const int f0 = 384 * w + 4 * t;
   const bool v0 = FULL || f0 < F, v1 = FULL || f0 + 128 < F, v2 = FULL || f0 + 256 < F;       // F % 4 == 0: whole 16-byte groups
@@ -179,7 +195,7 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
     c_next = sp.track_off[tr + 1];
     seg = max(cb, sp.track_off[tr]);               // first carrier index that can open a segment
   }
-  for (int i = tid; i < nw * F; i += blockDim.x) P[i] = 0.f;
+  for (int i = tid; i < p_floats; i += blockDim.x) P[i] = 0.f;
   __syncthreads();
   bool opened = false;
 
@@ -188,14 +204,14 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
     __syncthreads();
     for (int n = tid; n < nt; n += blockDim.x) {
       float s = 0.f;
-      for (int ww = 0; ww < nw; ++ww) {
-        const float* q = P + (size_t)ww * F + 3 * n;
+      for (int ww = 0; 128 * ww <= n; ++ww) {        // (warp ww holds S[g] for g >= 384 ww only; 128 ww <= n < nt keeps ww < nw)
+        const float* q = P + rows_offset(ww, F) - 384 * ww + 3 * n;
         s += (q[0] + q[1]) + q[2];
       }
       row[n] = s;
     }
     __syncthreads();
-    for (int i = tid; i < nw * F; i += blockDim.x) P[i] = 0.f;
+    for (int i = tid; i < p_floats; i += blockDim.x) P[i] = 0.f;
     __syncthreads();
   };
 
@@ -255,6 +271,8 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
           const NodeFrac nf = locate(p.pos[3 * s], p.pos[3 * s + 1], p.pos[3 * s + 2], p.nx, p.ny, p.nz, p.invx, p.invy, p.invz);
           const bool ok = nf.ok && isfinite(vx) && isfinite(vy) && isfinite(vz);
           unsigned key_hi = 0;
+          unsigned long long key = 0;
+          float wsk[8];
 #pragma unroll
           for (int k = 0; k < 8; ++k) {
             const int cx = k >> 2, cy = (k >> 1) & 1, cz = k & 1;
@@ -262,13 +280,37 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
             const int ix = cx ? nf.i1[0] : nf.i0[0], iy = cy ? nf.i1[1] : nf.i0[1], iz = cz ? nf.i1[2] : nf.i0[2];
             const unsigned node = ok ? (unsigned)((ix * p.ny + iy) * p.nz + iz) : 0u;
             const float ws = wgt * scale;            // a non-finite step contributes nothing (0, not 0 * inf)
-            tabc[js * 8 + k] = make_float2(__uint_as_float(node), ok ? ws : 0.f);
+            wsk[k] = ok ? ws : 0.f;
             if constexpr (CACHE) {
+              tabn[js * 8 + k] = node;
               if (k == 0) key_hi = node;
-              if (k == 7) keys[js] = ((unsigned long long)key_hi << 32) | node;   // corners 0 and 7 identify the cell (a skipped step has both 0: never a real cell)
+              if (k == 7) key = ((unsigned long long)key_hi << 32) | node;   // corners 0 and 7 identify the cell (a skipped step has both 0: never a real cell)
+            } else {
+              tabc[js * 8 + k] = make_float2(__uint_as_float(node), wsk[k]);
             }
           }
-          tabv[js] = ok ? make_float4(vx, vy, vz, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
+          if constexpr (CACHE) {
+            keys[js] = key;
+            // bit j of the change mask: step j + 1 of this table opens another cell than step j (taken as set across the
+            // 32-step words, where the neighbour's key is not at hand: the prefetch it triggers then asks for rows already near)
+            const unsigned act = __activemask();
+            const unsigned long long nk = __shfl_down_sync(act, key, 1);
+            const unsigned mw = __ballot_sync(act, (js + 1 < mc) && (t == 31 || nk != key));
+            if (t == 0) s_cmask[js >> 5] = mw;
+            const float v3[3] = {ok ? vx : 0.f, ok ? vy : 0.f, ok ? vz : 0.f};
+#pragma unroll
+            for (int rot = 0; rot < 3; ++rot) {
+              float q[24];
+#pragma unroll
+              for (int k = 0; k < 8; ++k)
+#pragma unroll
+                for (int cc = 0; cc < 3; ++cc) q[3 * k + cc] = wsk[k] * v3[(rot + cc) % 3];
+#pragma unroll
+              for (int i = 0; i < 6; ++i) tabq[(js * 3 + rot) * 6 + i] = make_float4(q[4 * i], q[4 * i + 1], q[4 * i + 2], q[4 * i + 3]);
+            }
+          } else {
+            tabv[js] = ok ? make_float4(vx, vy, vz, 0.f) : make_float4(0.f, 0.f, 0.f, 0.f);
+          }
         }
         __syncthreads();
         for (int jm = 0; jm < mc; ++jm) {
@@ -280,21 +322,32 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
               cell_key = key;
 #pragma unroll
               for (int k = 0; k < 8; ++k) {
-                const float* __restrict__ src = p.H + (size_t)__float_as_uint(tabc[jm * 8 + k].x) * F + f0;
+                const float* __restrict__ src = p.H + (size_t)tabn[jm * 8 + k] * F + f0;
                 HC[k][0] = v0 ? ldg4(src) : z4; HC[k][1] = v1 ? ldg4(src + 128) : z4; HC[k][2] = v2 ? ldg4(src + 256) : z4;
               }
-            }
-            const float4 vv = tabv[jm];
-            const float q0 = r0 ? vv.x : (r1 ? vv.y : vv.z);      // velocity component (t + x) % 3, x = 0, 1, 2
-            const float q1 = r0 ? vv.y : (r1 ? vv.z : vv.x);
-            const float q2 = r0 ? vv.z : (r1 ? vv.x : vv.y);
-            const float4* tc4 = reinterpret_cast<const float4*>(tabc + jm * 8);
+              {
+                // the next cell of this table is asked into L2 now: its rows arrive while the steps inside this cell are
+                // summed (tables beyond L2: +10 % at configs[4]).  A warp's share of 8 rows is 8 x 12 lines of 128 bytes:
+                // three per lane.
+                const unsigned word = s_cmask[jm >> 5] >> (jm & 31);
+                const int jn = jm + __ffs(word);
+                if (word != 0 && jn < mc) {
 #pragma unroll
-            for (int kk = 0; kk < 4; ++kk) {
-              const float4 e2 = tc4[kk];             // (node, w * scale) of corners 2 kk and 2 kk + 1
-              fma12q(A, e2.y * q0, e2.y * q1, e2.y * q2, HC[2 * kk][0], HC[2 * kk][1], HC[2 * kk][2]);
-              fma12q(A, e2.w * q0, e2.w * q1, e2.w * q2, HC[2 * kk + 1][0], HC[2 * kk + 1][1], HC[2 * kk + 1][2]);
+                  for (int i = 0; i < 3; ++i) {
+                    const int idx = t + 32 * i, k = idx / 12, l = idx - 12 * k;
+                    const int fo = 384 * w + 32 * l;
+                    const float* a = p.H + (size_t)tabn[jn * 8 + k] * F + fo;
+                    if (FULL || fo < F) asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
+                  }
+                }
+              }
             }
+            const float4* tq = tabq + (jm * 3 + r) * 6;
+            float q[24];
+#pragma unroll
+            for (int i = 0; i < 6; ++i) { const float4 e = tq[i]; q[4 * i] = e.x; q[4 * i + 1] = e.y; q[4 * i + 2] = e.z; q[4 * i + 3] = e.w; }
+#pragma unroll
+            for (int k = 0; k < 8; ++k) fma12q(A, q[3 * k], q[3 * k + 1], q[3 * k + 2], HC[k][0], HC[k][1], HC[k][2]);
           } else {
             const float4 vv = tabv[jm];
             const float q0 = r0 ? vv.x : (r1 ? vv.y : vv.z);      // velocity component (t + x) % 3, x = 0, 1, 2
@@ -442,7 +495,8 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
     if (const char* ev = std::getenv("WTIDE_CONV_CACHE")) cache = ev[0] == '1';
     const bool full = g->nt % 128 == 0;
     auto fn = cache ? (full ? k_conv_systolic<true, true> : k_conv_systolic<true, false>) : (full ? k_conv_systolic<false, true> : k_conv_systolic<false, false>);
-    const size_t smem = (size_t)(cache ? kStepChunkCached : kStepChunk) * 8 * sizeof(float4) + (size_t)nw * 3 * g->nt * sizeof(float);
+    const size_t smem = (cache ? (size_t)kStepChunkCached * kStepBytesCached : (size_t)kStepChunk * kStepBytesPlain) +
+                        (size_t)rows_offset(nw, 3 * g->nt) * sizeof(float);
     cudaError_t ea = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (ea != cudaSuccess) { wt_set_error(std::string("wt_convolve_currents: ") + cudaGetErrorString(ea)); return WT_ECUDA; }
     ++g_wt_launches;
