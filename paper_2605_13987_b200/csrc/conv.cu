@@ -154,10 +154,13 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
   const int nt = p.nt, F = 3 * nt;
   const int tid = threadIdx.x, w = tid >> 5, t = tid & 31, nw = blockDim.x >> 5;
   extern __shared__ __align__(16) unsigned char smraw[];
-  // partial rows: warp w only ever holds sums S[g], g >= 384 w, so its row is the F - 384 w floats [384 w, F)
+  // BAL (cached kernel): the (lag block, step) pairs of a step table are dealt out evenly to the warps, see below; a warp then
+  // holds sums of any block and its partial row is all F floats.  Otherwise warp w owns block w and only ever holds sums
+  // S[g], g >= 384 w: its row is the F - 384 w floats [384 w, F).
+  constexpr bool BAL = CACHE;
   float* P = reinterpret_cast<float*>(smraw + CH * kStepBytes);
-  float* Pw = P + rows_offset(w, F) - 384 * w;                          // Pw[g], 384 w <= g < F
-  const int p_floats = rows_offset(nw, F);
+  float* Pw = BAL ? P + (size_t)w * F : P + rows_offset(w, F) - 384 * w;    // Pw[g]
+  const int p_floats = BAL ? nw * F : rows_offset(nw, F);
   __shared__ int64_t s_track;
   __shared__ unsigned s_cmask[kStepChunkCached / 32];   // cached kernel: where the carrier changes cell inside the step table
   // step table: per step eight (node, w * scale) pairs, the velocity and (CACHE) the cell key
@@ -170,8 +173,6 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
   unsigned* tabn = reinterpret_cast<unsigned*>(smraw + CH * 3 * 24 * sizeof(float));                       // [CH][8]
   if constexpr (CACHE) keys = reinterpret_cast<unsigned long long*>(smraw + CH * (3 * 24 * sizeof(float) + 8 * sizeof(unsigned)));
 
-  const int f0 = 384 * w + 4 * t;
-  const bool v0 = FULL || f0 < F, v1 = FULL || f0 + 128 < F, v2 = FULL || f0 + 256 < F;       // F % 4 == 0: whole 16-byte groups
   const int r = t % 3;
   const bool r0 = (r == 0), r1 = (r == 1);
 
@@ -204,8 +205,8 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
     __syncthreads();
     for (int n = tid; n < nt; n += blockDim.x) {
       float s = 0.f;
-      for (int ww = 0; 128 * ww <= n; ++ww) {        // (warp ww holds S[g] for g >= 384 ww only; 128 ww <= n < nt keeps ww < nw)
-        const float* q = P + rows_offset(ww, F) - 384 * ww + 3 * n;
+      for (int ww = 0; BAL ? ww < nw : 128 * ww <= n; ++ww) {   // (!BAL: warp ww holds S[g] for g >= 384 ww only; 128 ww <= n < nt keeps ww < nw)
+        const float* q = (BAL ? P + (size_t)ww * F : P + rows_offset(ww, F) - 384 * ww) + 3 * n;
         s += (q[0] + q[1]) + q[2];
       }
       row[n] = s;
@@ -235,9 +236,9 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
       for (int i = 0; i < 4; ++i) A[j][i] = 0.f;
 
     // m -> m + 1: the sums move down by three floats; the three lowest of the warp are complete
-    auto shift = [&](int m) {
+    auto shift = [&](int u, int m) {
       if (t == 0) {
-        const int gq = 384 * w + 3 * m;
+        const int gq = 384 * u + 3 * m;
         if (gq < F) { Pw[gq] += A[0][0]; Pw[gq + 1] += A[0][1]; Pw[gq + 2] += A[0][2]; }   // F % 3 == 0
       }
       float sh[3][3];
@@ -313,9 +314,37 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
           }
         }
         __syncthreads();
-        for (int jm = 0; jm < mc; ++jm) {
+        // Lag block u (floats [384 u, 384 u + 384) of the rows) has outputs below nt for the steps m < nt - 128 u only (the causal
+        // triangle): with one block per warp, warp nw - 1 is done after 128 steps, the next after 256, ... and their schedulers
+        // idle.  BAL: the live (block, step) pairs of this table, block-major, are cut into nw equal runs, one per warp; a warp
+        // starts each of its (at most three) pieces with empty sums and leaves them in its own row at the end of the piece, so
+        // the result depends on nt, M and nw only (R25).  A table of a carrier's first 128 steps gives warp w block w as before.
+        int lo = 0, hi = mc;
+        if constexpr (BAL) {
+          int total = 0;
+          for (int u = 0; u < nw; ++u) total += max(0, min(mc, nt - 128 * u - m0));
+          const int per = (total + nw - 1) / nw;
+          lo = w * per; hi = min(total, lo + per);
+        }
+        int base = 0;
+        for (int u = BAL ? 0 : w; u < (BAL ? nw : w + 1); ++u) {
+        const int len = BAL ? max(0, min(mc, nt - 128 * u - m0)) : mc;
+        const int ja = BAL ? max(lo, base) - base : 0, jb = BAL ? min(hi, base + len) - base : mc;
+        base += len;
+        if (ja >= jb) continue;
+        const int f0 = 384 * u + 4 * t;
+        const bool v0 = FULL || f0 < F, v1 = FULL || f0 + 128 < F, v2 = FULL || f0 + 256 < F;       // F % 4 == 0: whole 16-byte groups
+        if constexpr (BAL) {
+#pragma unroll
+          for (int j = 0; j < 3; ++j)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) A[j][i] = 0.f;
+          cell_key = ~0ULL;
+        }
+        int jm = ja;
+        for (; jm < jb; ++jm) {
           const int m = m0 + jm;
-          if (128 * w + m >= nt) break;              // every output of this warp is past nt from here on (warp uniform)
+          if (128 * u + m >= nt) break;              // every output of this block is past nt from here on (warp uniform)
           if constexpr (CACHE) {
             const unsigned long long key = keys[jm];
             if (key != cell_key) {                   // (warp uniform)
@@ -335,7 +364,7 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
 #pragma unroll
                   for (int i = 0; i < 3; ++i) {
                     const int idx = t + 32 * i, k = idx / 12, l = idx - 12 * k;
-                    const int fo = 384 * w + 32 * l;
+                    const int fo = 384 * u + 32 * l;
                     const float* a = p.H + (size_t)tabn[jn * 8 + k] * F + fo;
                     if (FULL || fo < F) asm volatile("prefetch.global.L2 [%0];" ::"l"(a));
                   }
@@ -369,20 +398,36 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
               }
             }
           }
-          shift(m);
+          shift(u, m);
+        }
+        if constexpr (BAL) {
+          // after the steps [m0 + ja, m0 + jm) lane (j, i) holds its share of S[f + 3 (m0 + jm)]
+          __syncwarp();
+#pragma unroll
+          for (int j = 0; j < 3; ++j)
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const int gq = f0 + 128 * j + i + 3 * (m0 + jm);
+              if (f0 + 128 * j < F && gq < F) Pw[gq] += A[j][i];
+            }
+          __syncwarp();
+        }
         }
       }
     }
-    // after M steps lane (j, i) holds S[f + 3 M]
-    __syncwarp();
+    if constexpr (!BAL) {
+      // after M steps lane (j, i) holds S[f + 3 M]
+      const int f0 = 384 * w + 4 * t;
+      __syncwarp();
 #pragma unroll
-    for (int j = 0; j < 3; ++j)
+      for (int j = 0; j < 3; ++j)
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        const int gq = f0 + 128 * j + i + 3 * M;
-        if (f0 + 128 * j < F && gq < F) Pw[gq] += A[j][i];   // (a warp that left the loop early holds outputs >= nt only)
-      }
-    __syncwarp();
+        for (int i = 0; i < 4; ++i) {
+          const int gq = f0 + 128 * j + i + 3 * M;
+          if (f0 + 128 * j < F && gq < F) Pw[gq] += A[j][i];   // (a warp that left the loop early holds outputs >= nt only)
+        }
+      __syncwarp();
+    }
     if (!sp.per_track) flush_row(p.out + (size_t)c * nt);
   }
   if (sp.per_track && opened) flush_row(p.out + (size_t)seg * nt);
@@ -496,7 +541,7 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
     const bool full = g->nt % 128 == 0;
     auto fn = cache ? (full ? k_conv_systolic<true, true> : k_conv_systolic<true, false>) : (full ? k_conv_systolic<false, true> : k_conv_systolic<false, false>);
     const size_t smem = (cache ? (size_t)kStepChunkCached * kStepBytesCached : (size_t)kStepChunk * kStepBytesPlain) +
-                        (size_t)rows_offset(nw, 3 * g->nt) * sizeof(float);
+                        (size_t)(cache ? nw * 3 * g->nt : rows_offset(nw, 3 * g->nt)) * sizeof(float);
     cudaError_t ea = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (ea != cudaSuccess) { wt_set_error(std::string("wt_convolve_currents: ") + cudaGetErrorString(ea)); return WT_ECUDA; }
     ++g_wt_launches;
