@@ -118,11 +118,12 @@ __global__ void __launch_bounds__(kThreads) k_conv_carrier(ConvParams p) {
 // a corner are rotated by t % 3 once per corner with selects.
 // One CTA handles `gc` consecutive carriers; with per_track the rows of carriers of one track are
 // summed in P (carrier order) and written as one partial row at the index of the segment's first carrier.
-// grid = ceil(n_carriers / gc), block = 32 * ceil(nt / 128) <= 256,
+// grid = ceil(n_carriers / gc), block = 32 * ceil(nt / 128) <= 256 (cached kernel: 384, as many warps as have a partial row in 220 KB),
 // dynamic smem = step table (32 steps of 128 bytes; cached kernel 128 steps of 328 bytes) + the partial rows, warp w's being
 // the F - 384 w floats it can reach (55 KB instead of 98 KB at nt = 1024, which goes to L1).
 // ------------------------------------------------------------------------------------------------
 constexpr int kStepChunk = 32;        // steps per step table: plain kernel (carriers of a few dozen steps)
+constexpr int kCachedThreads = 384;   // cached kernel: twelve warps share the eight lag blocks of nt = 1024 (162 registers, one CTA per SM)
 constexpr int kStepChunkCached = 128;  // cached kernel (nt >= 1024, hundreds of steps: fewer table builds, during which seven warps wait)
 
 // shared memory of the systolic kernel: bytes per step of the step table, and the float offset of warp w's partial row
@@ -147,12 +148,13 @@ __device__ __forceinline__ float4 ldg4(const float* p) { return __ldg(reinterpre
 // FULL: nt is a multiple of 128, so every lane of every warp owns three whole 16-byte groups of a row and the row loads need no
 // predicates (all BASELINE configs).
 template <bool CACHE, bool FULL>
-__global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams sp) {
+__global__ void __launch_bounds__(CACHE ? kCachedThreads : 256, CACHE ? 1 : 2) k_conv_systolic(SysParams sp) {
   constexpr int CH = CACHE ? kStepChunkCached : kStepChunk;
   constexpr int kStepBytes = CACHE ? kStepBytesCached : kStepBytesPlain;
   const ConvParams& p = sp.c;
   const int nt = p.nt, F = 3 * nt;
-  const int tid = threadIdx.x, w = tid >> 5, t = tid & 31, nw = blockDim.x >> 5;
+  const int tid = threadIdx.x, w = tid >> 5, t = tid & 31, nw = blockDim.x >> 5;     // nw warps
+  const int nb = (nt + 127) >> 7;                                                        // nb lag blocks of 128 lags (= nw unless BAL)
   extern __shared__ __align__(16) unsigned char smraw[];
   // BAL (cached kernel): the (lag block, step) pairs of a step table are dealt out evenly to the warps, see below; a warp then
   // holds sums of any block and its partial row is all F floats.  Otherwise warp w owns block w and only ever holds sums
@@ -318,16 +320,16 @@ __global__ void __launch_bounds__(256, CACHE ? 1 : 2) k_conv_systolic(SysParams 
         // triangle): with one block per warp, warp nw - 1 is done after 128 steps, the next after 256, ... and their schedulers
         // idle.  BAL: the live (block, step) pairs of this table, block-major, are cut into nw equal runs, one per warp; a warp
         // starts each of its (at most three) pieces with empty sums and leaves them in its own row at the end of the piece, so
-        // the result depends on nt, M and nw only (R25).  A table of a carrier's first 128 steps gives warp w block w as before.
+        // the result depends on nt, M and nw only (R25).  The CTA has more warps than blocks (twelve for the eight blocks of nt = 1024).
         int lo = 0, hi = mc;
         if constexpr (BAL) {
           int total = 0;
-          for (int u = 0; u < nw; ++u) total += max(0, min(mc, nt - 128 * u - m0));
+          for (int u = 0; u < nb; ++u) total += max(0, min(mc, nt - 128 * u - m0));
           const int per = (total + nw - 1) / nw;
           lo = w * per; hi = min(total, lo + per);
         }
         int base = 0;
-        for (int u = BAL ? 0 : w; u < (BAL ? nw : w + 1); ++u) {
+        for (int u = BAL ? 0 : w; u < (BAL ? nb : w + 1); ++u) {
         const int len = BAL ? max(0, min(mc, nt - 128 * u - m0)) : mc;
         const int ja = BAL ? max(lo, base) - base : 0, jb = BAL ? min(hi, base + len) - base : mc;
         base += len;
@@ -540,13 +542,20 @@ extern "C" int wt_convolve_currents(const wt_geometry* g, const float* H_dev, in
     if (const char* ev = std::getenv("WTIDE_CONV_CACHE")) cache = ev[0] == '1';
     const bool full = g->nt % 128 == 0;
     auto fn = cache ? (full ? k_conv_systolic<true, true> : k_conv_systolic<true, false>) : (full ? k_conv_systolic<false, true> : k_conv_systolic<false, false>);
+    // cached kernel: warps beyond the nw lag blocks (its work is dealt out per (block, step)); each needs a full partial row
+    int warps = nw;
+    if (cache) {
+      warps = kCachedThreads / 32;
+      const size_t row = (size_t)3 * g->nt * sizeof(float), room = 220 * 1024 - (size_t)kStepChunkCached * kStepBytesCached;
+      warps = (int)std::max<size_t>(1, std::min<size_t>(warps, room / row));
+    }
     const size_t smem = (cache ? (size_t)kStepChunkCached * kStepBytesCached : (size_t)kStepChunk * kStepBytesPlain) +
-                        (size_t)(cache ? nw * 3 * g->nt : rows_offset(nw, 3 * g->nt)) * sizeof(float);
+                        (size_t)(cache ? warps * 3 * g->nt : rows_offset(nw, 3 * g->nt)) * sizeof(float);
     cudaError_t ea = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (ea != cudaSuccess) { wt_set_error(std::string("wt_convolve_currents: ") + cudaGetErrorString(ea)); return WT_ECUDA; }
     ++g_wt_launches;
     const int64_t sg = (int64_t)gc * stride;
-    fn<<<(unsigned)((n_carriers + sg - 1) / sg * stride), 32 * nw, smem, st>>>(sp);
+    fn<<<(unsigned)((n_carriers + sg - 1) / sg * stride), 32 * warps, smem, st>>>(sp);
   } else if (n_carriers > 0) {
     ++g_wt_launches;
     k_conv_carrier<<<(unsigned)n_carriers, kThreads, 0, st>>>(p);
