@@ -271,3 +271,31 @@ def test_row_cache_kernel_and_plain_kernel_agree_with_the_oracle(cache, monkeypa
             ref = _oracle(d, Hnp, csr, per_track)
             assert np.isfinite(got).all()
             assert np.abs(got - ref).max() <= TOL * np.abs(ref).max(), (nt, per_track)
+
+
+@pytest.mark.parametrize("nt", [1024, 896, 1000, 260])
+def test_long_carriers_share_the_causal_triangle(nt, monkeypatch):
+    """Cached kernel: the (lag block, step) pairs of every 128-step table are dealt out evenly to the warps (more warps than
+    blocks), pieces start with empty sums.  Carriers of 127 ... nt + 300 steps (tables at which 0 ... all but one block have
+    run past nt, a ragged last table), nt a multiple of 128 or not, against the oracle; twice for the same bits (R25)."""
+    monkeypatch.setenv("WTIDE_CONV_CACHE", "1")
+    d = reduced_desc(geometry_desc(0), grid=(12, 8, 6), nt=nt)
+    g = wt.wt_make_geometry(d)
+    rng = np.random.default_rng(200 + nt)
+    Hnp = rng.standard_normal((12, 8, 6, nt, 3)).astype(np.float32)
+    H = torch.as_tensor(Hnp).to(DEV)
+    cell = np.array([d["lx"] / 12, d["ly"] / 8, d["lz"] / 6])
+    lens = [127, 128, 129, 300, min(640, nt - 1), nt, nt + 300, 2, 385]
+    off = np.concatenate([[0], np.cumsum(lens)]).astype(np.int64)
+    pos = np.concatenate([rng.uniform(0, 1, 3) * np.array([d["lx"], d["ly"], d["lz"]]) + np.cumsum(rng.normal(0, 0.2, size=(n, 3)) * cell, axis=0)
+                          for n in lens]).astype(np.float32)
+    vel = rng.standard_normal((int(off[-1]), 3)).astype(np.float32)
+    csr = dict(track_carrier_offsets=np.array([0, 4, 7, 9], np.int64), carrier_step_offsets=off, pos=pos, vel=vel,
+               charge=rng.standard_normal(len(lens)).astype(np.float32))
+    for per_track in (False, True):
+        got = _run(g, H, csr, per_track)
+        ref = _oracle(d, Hnp, csr, per_track)
+        assert np.isfinite(got).all()
+        assert np.abs(got - ref).max() <= TOL * np.abs(ref).max(), (nt, per_track)
+        again = _run(g, H, csr, per_track)
+        assert np.array_equal(got.view(np.uint32), again.view(np.uint32))
