@@ -238,10 +238,17 @@ __global__ void __launch_bounds__(CACHE ? kCachedThreads : 256, CACHE ? 1 : 2) k
       for (int i = 0; i < 4; ++i) A[j][i] = 0.f;
 
     // m -> m + 1: the sums move down by three floats; the three lowest of the warp are complete
+    // (lane 0 reads the three sums it will complete at the top of the step, pre(), and writes them back in shift(): the shared
+    // load is then not waited for behind the step's 96 FMA)
+    float pq[3] = {0.f, 0.f, 0.f};
+    auto pre = [&](int u, int m) {
+      const int gq = 384 * u + 3 * m;
+      if (t == 0 && gq < F) { pq[0] = Pw[gq]; pq[1] = Pw[gq + 1]; pq[2] = Pw[gq + 2]; }     // F % 3 == 0
+    };
     auto shift = [&](int u, int m) {
-      if (t == 0) {
+      {
         const int gq = 384 * u + 3 * m;
-        if (gq < F) { Pw[gq] += A[0][0]; Pw[gq + 1] += A[0][1]; Pw[gq + 2] += A[0][2]; }   // F % 3 == 0
+        if (t == 0 && gq < F) { Pw[gq] = pq[0] + A[0][0]; Pw[gq + 1] = pq[1] + A[0][1]; Pw[gq + 2] = pq[2] + A[0][2]; }
       }
       float sh[3][3];
 #pragma unroll
@@ -347,6 +354,7 @@ __global__ void __launch_bounds__(CACHE ? kCachedThreads : 256, CACHE ? 1 : 2) k
         for (; jm < jb; ++jm) {
           const int m = m0 + jm;
           if (128 * u + m >= nt) break;              // every output of this block is past nt from here on (warp uniform)
+          pre(u, m);
           if constexpr (CACHE) {
             const unsigned long long key = keys[jm];
             if (key != cell_key) {                   // (warp uniform)
